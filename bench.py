@@ -1,0 +1,317 @@
+#!/usr/bin/env python
+"""bench.py — MLUPS of the fused D3Q27 Reg-FLBM collide-stream step on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W]            # this repository's CUDA path
+    python bench.py --impl reference [--steps K] [--warmup W]      # the CPU oracle, timed as it stands
+
+A "step" is one time step of Eq.24 over the whole lattice: one launch of the fused
+pull-stream + collide kernel.  Workload at N=1: BASELINE.json configs[3] — 512^3 periodic, fp64, tau=0.8,
+kT=1e-4, seed 11, rho0=1, u=0 (the configuration the MLUPS metric is quoted on; 58 GB A-B workspace).
+With --gpus N (torchrun, one rank per GPU) every rank runs an independent replica of that lattice
+("replicas only": BASELINE.json fixes one GPU with no sharding and no collectives);
+value = sites updated by all ranks / max-over-ranks device time.
+
+One JSON line is printed by rank 0.  value: device-resident throughput (CUDA events on the launching stream
+around K steps); e2e: the same metric through rflbm_run_host with HOST (pinned) buffers, H2D of (rho,u),
+K steps, D2H of the moments all inside the timed region; roofline: algorithmic bytes (2*27*8 B per site)
+over the average launch time vs the measured HBM peak; cpu_baseline: the oracle on this box's host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "MLUPS per B200 (fp64 D3Q27 Reg-FLBM)"
+UNIT = "MLUPS"
+WORKLOAD = dict(size=512, tau=0.8, kT=1e-4, seed=11, rho0=1.0)
+FALLBACK_HBM_GBS = 6650.0      # /opt/skills/guides/B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
+
+
+def parse_args():
+    p = argparse.ArgumentParser()
+    p.add_argument("--gpus", type=int, default=1)
+    p.add_argument("--steps", type=int, default=200)
+    p.add_argument("--warmup", type=int, default=10)
+    p.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    # development knobs (the driver does not pass them)
+    p.add_argument("--size", type=int, default=WORKLOAD["size"])
+    p.add_argument("--kT", type=float, default=WORKLOAD["kT"])
+    p.add_argument("--precision", default="f64", choices=["f64", "f32"])
+    p.add_argument("--no-e2e", action="store_true")
+    p.add_argument("--no-cpu", action="store_true")
+    p.add_argument("--cpu-seconds", type=float, default=12.0)
+    return p.parse_args()
+
+
+# ----------------------------------------------------------------------------- helpers
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100", "-i", str(self.index)], stdout=subprocess.PIPE, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [t.strip() for t in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def hbm_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic_bytes(size, precision):
+    """dram bytes per launch of the step kernel from the committed ncu --set full summary, if any."""
+    path = os.path.join(ROOT, "profiles", f"step_kernel_traffic_{size}_{precision}.txt")
+    try:
+        with open(path) as fh:
+            for line in fh:
+                if line.startswith("dram_bytes_per_launch="):
+                    return float(line.split("=", 1)[1])
+    except OSError:
+        pass
+    return None
+
+
+def dist_setup(n_gpus):
+    """(rank, world, local_rank); initialises NCCL when launched by torchrun."""
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29500")
+        import torch
+        backend = "nccl" if torch.cuda.is_available() else "gloo"
+        dist.init_process_group(backend, rank=rank, world_size=world)
+    return rank, world, local
+
+
+def barrier_all():
+    import torch.distributed as dist
+    if dist.is_available() and dist.is_initialized():
+        dist.barrier()
+
+
+def max_over_ranks(value, device=None):
+    """max over all ranks of a python float (device time in ms): the job finishes when the slowest rank does."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()):
+        return float(value)
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def sum_over_ranks(value, device=None):
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()):
+        return float(value)
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return float(t.item())
+
+
+# ----------------------------------------------------------------------------- CPU oracle leg
+def time_oracle(steps, warmup, seconds=None, size=64):
+    """Oracle as it stands on the host cores: `size`^3 sample of the workload, all cores (OpenMP over z)."""
+    import oracle
+    cores = oracle.max_threads()
+    ref = oracle.Ref(size, size, size, WORKLOAD["tau"], WORKLOAD["kT"], WORKLOAD["rho0"], WORKLOAD["seed"],
+                     threads=cores)
+    ref.init()
+    ref.step(max(1, warmup))
+    if seconds is not None:                      # bounded: choose the step count for ~`seconds` of CPU work
+        t0 = time.perf_counter(); ref.step(2); dt = (time.perf_counter() - t0) / 2
+        steps = max(2, min(steps, int(seconds / max(dt, 1e-6))))
+    t0 = time.perf_counter()
+    ref.step(steps)
+    dt = time.perf_counter() - t0
+    mlups = size ** 3 * steps / dt / 1e6
+    return mlups, cores, steps, dt, f"{size}^3 periodic sub-lattice of the workload (same tau, kT, seed), {steps} steps"
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    size = 64
+    mlups, cores, steps, dt, sample = time_oracle(args.steps, args.warmup, seconds=None, size=size)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": mlups, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+        "warmup": args.warmup, "ms_per_step": dt / steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "512^3 periodic D3Q27 Reg-FLBM fp64, tau=0.8, kT=1e-4, seed 11 (BASELINE configs[3]); "
+                               "each step = one oracle time step on a 64^3 sample of it", "l2": "n/a (CPU)"},
+        "cpu_baseline": {"value": mlups, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": mlups, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ----------------------------------------------------------------------------- CUDA leg
+def run_ours(args):
+    import torch
+    from paper_2507_08820_b200 import binding
+
+    rank, world, local = dist_setup(args.gpus)
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: CUDA is not available and the rflbm path has no CPU fallback")
+    dev = torch.device(f"cuda:{local}")
+    torch.cuda.set_device(dev)
+    n = args.size
+    prec = binding.F64 if args.precision == "f64" else binding.F32
+    es = 8 if prec == binding.F64 else 4
+    N = n ** 3
+    K, W = args.steps, max(3, args.warmup)
+
+    sim = binding.Rflbm(n, n, n, WORKLOAD["tau"], args.kT, WORKLOAD["rho0"], WORKLOAD["seed"], prec, device=dev)
+    sim.init()
+    sim.step(W)                                     # warm-up: also thermalises the state
+    torch.cuda.synchronize(dev)
+
+    # ---- device-resident timing: K launches of the step kernel, CUDA events on the launching stream
+    stream = sim.stream
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    vis = [v for v in os.environ.get("CUDA_VISIBLE_DEVICES", "").split(",") if v.strip()]
+    sampler = ClockSampler(vis[local] if local < len(vis) else local)
+    l0 = sim.launch_count
+    barrier_all(); torch.cuda.synchronize(dev)
+    if rank == 0:
+        sampler.start()
+    ev0.record(stream)
+    sim.step(K)
+    ev1.record(stream)
+    torch.cuda.synchronize(dev); barrier_all()
+    clocks = sampler.stop() if rank == 0 else None
+    ms_local = ev0.elapsed_time(ev1)
+    launches = sim.launch_count - l0
+    ms = max_over_ranks(ms_local, dev)
+    value = N * K * world / (ms * 1e-3) / 1e6
+
+    # conservation after the run (cheap sanity on the timed state)
+    d = sim.diagnostics()
+    mass_err = abs(d[0] / N / WORKLOAD["rho0"] - 1.0)
+
+    # ---- end to end through the C-ABI with HOST buffers
+    e2e = None
+    if not args.no_e2e:
+        shape = (n, n, n)
+        dt = torch.float64 if prec == binding.F64 else torch.float32
+        rho_h = torch.full(shape, WORKLOAD["rho0"], dtype=dt).pin_memory()
+        u_h = torch.zeros((3,) + shape, dtype=dt).pin_memory()
+        rho_o = torch.empty(shape, dtype=dt).pin_memory()
+        u_o = torch.empty((3,) + shape, dtype=dt).pin_memory()
+        scratch = torch.empty(4 * N * es, dtype=torch.uint8, device=dev)
+        sim.run_host(rho_h, u_h, 2, rho_o, u_o, scratch)              # warm the copy path
+        barrier_all(); torch.cuda.synchronize(dev)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        sim.run_host(rho_h, u_h, K, rho_o, u_o, scratch)              # H2D + init + K steps + moments + D2H + sync
+        e1.record(stream)
+        torch.cuda.synchronize(dev); barrier_all()
+        ms_e = max_over_ranks(e0.elapsed_time(e1), dev)
+        e2e = {"value": N * K * world / (ms_e * 1e-3) / 1e6, "unit": UNIT,
+               "h2d_bytes_per_step": 4 * N * es / K, "d2h_bytes_per_step": 4 * N * es / K,
+               "ms_total": ms_e, "what": "rflbm_run_host: pinned host rho,u -> device, init, K steps, moments, "
+                                         "device -> pinned host, stream sync; bytes are per job / K"}
+        assert abs(float(rho_o.double().mean()) / WORKLOAD["rho0"] - 1.0) < 1e-9
+        del rho_h, u_h, rho_o, u_o, scratch
+
+    if rank != 0:
+        return 0
+
+    peak, peak_src = hbm_peak()
+    bytes_per_launch = 2 * 27 * es * N
+    achieved = bytes_per_launch / (ms_local / K * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": ncu_traffic_bytes(n, args.precision), "peak_source": peak_src,
+                "kernel": "step_kernel", "algorithmic_bytes_per_launch": bytes_per_launch,
+                "avg_launch_ms": ms_local / K}
+
+    cpu = None
+    if not args.no_cpu:
+        mlups, cores, csteps, cdt, sample = time_oracle(10 ** 6, 1, seconds=args.cpu_seconds, size=64)
+        cpu = {"value": mlups, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample, "seconds": cdt}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": args.precision, "data": "synthetic",
+        "config": {"workload": f"{n}^3 periodic D3Q27 Reg-FLBM {args.precision}, rho0=1, u=0, tau=0.8, kT={args.kT:g}, "
+                               f"seed 11 (BASELINE configs[3]); A-B double buffer {2 * 27 * es * N / 1e9:.1f} GB",
+                   "l2": "no flush needed: each step streams 2*27*N*sizeof(real) bytes >> 126 MB L2",
+                   "parallelism": "replicas only" if world > 1 else "single GPU"},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
+        "hbm_gbs": achieved, "mass_rel_err": mass_err,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

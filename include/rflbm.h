@@ -1,0 +1,110 @@
+/*
+ * rflbm.h — C-ABI boundary of the B200-native D3Q27 regularized fluctuating lattice Boltzmann
+ * (Reg-FLBM) collide-and-stream path of arXiv 2507.08820.
+ *
+ * Citations are PAPER.md line : equation.  "R<n>" are the readings listed in DESIGN.md.
+ *
+ * Conventions (all entry points)
+ *   - Every function returns RFLBM_OK (0) or a negative code; none throws or aborts.  After a failure
+ *     rflbm_last_error(h) returns a NUL-terminated description owned by the handle.
+ *   - Pointers named *_dev are DEVICE pointers, *_host are HOST pointers.  The library NEVER allocates
+ *     device memory and NEVER creates streams: the caller (PyTorch in this repository) owns both and
+ *     must keep them alive for as long as the handle uses them (borrowed, never freed by the library).
+ *   - Field layout: x fastest, site index s = x + nx*(y + ny*z); structure of arrays by component:
+ *     rho[N], u[3][N], f[27][N] with N = nx*ny*nz.  Element type `real` = double (RFLBM_F64) or float
+ *     (RFLBM_F32, fp32 population storage and fp32 arithmetic, R14).
+ *   - Population order at the boundary ("canonical", R1): 0:(0,0,0); 1..6: +x,-x,+y,-y,+z,-z;
+ *     7..10: (sx,sy,0); 11..14: (sx,0,sz); 15..18: (0,sy,sz) with (s1,s2) = (+,+),(+,-),(-,+),(-,-);
+ *     19..26: (sx,sy,sz), sx outermost, sign order +,-.
+ *   - Observable state (R10): the PRE-collision populations f_i(x,t) of Eq.1 after t steps;
+ *     the internal storage (post-collision, un-streamed, A-B double buffer) is not exposed.
+ *   - All work is enqueued on the stream given by rflbm_set_stream (default: the legacy stream 0) and is
+ *     asynchronous unless stated otherwise.
+ */
+#ifndef RFLBM_H
+#define RFLBM_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rflbm rflbm_t; /* opaque host-side handle */
+
+enum { RFLBM_F64 = 0, RFLBM_F32 = 1 };
+enum { RFLBM_OK = 0, RFLBM_EINVAL = -1, RFLBM_ESTATE = -2, RFLBM_ENOMEM = -3, RFLBM_ECUDA = -4 };
+
+/* Problem definition: lattice size, hydrodynamic relaxation time tau_h = 1/omega_h (nu = (tau-1/2)/3,
+ * PAPER.md:52; ghost rate omega_g = 1, :215), thermal energy kT (Eq.9 :99; kT = 0 -> deterministic
+ * Reg-LBM, :294), reference density rho0 (:252), Philox seed (R8) and precision.
+ * Host only: no GPU work, no allocation on the device.
+ * EINVAL: nx,ny,nz < 1, N >= 2^32, tau <= 0.5 or non-finite, kT < 0, rho0 <= 0, unknown precision, out NULL. */
+int rflbm_create(int nx, int ny, int nz, double tau, double kT, double rho0, uint64_t seed, int precision,
+                 rflbm_t** out);
+
+/* Bytes of device workspace the handle needs: two population buffers 2*27*N*sizeof(real) (A-B scheme)
+ * plus a 4 KiB reduction scratch and 8 KiB of Box-Muller tables (uploaded here, synchronously). */
+size_t rflbm_workspace_bytes(const rflbm_t* h);
+
+/* Borrow `bytes` of device memory at dev_ptr (256-byte aligned) as the workspace.
+ * ENOMEM if too small or misaligned.  Invalidates the state (rflbm_init / rflbm_set_populations needed). */
+int rflbm_set_workspace(rflbm_t* h, void* dev_ptr, size_t bytes);
+
+/* cudaStream_t (as void*) on which every later call enqueues its work; borrowed. */
+int rflbm_set_stream(rflbm_t* h, void* cuda_stream);
+
+/* Solid layers z=0 and z=nz-1 with halfway bounce-back (R12; not in the paper, whose runs are periodic, :252).
+ * Default off (periodic in x,y,z).  EINVAL if nz < 3.  Must be called before init/set_populations. */
+int rflbm_set_walls_z(rflbm_t* h, int on);
+
+/* Uniform acceleration g: body force F = rho*g, Guo forcing in moment form (R13).  Default 0. */
+int rflbm_set_force(rflbm_t* h, double gx, double gy, double gz);
+
+/* f = f^(0)(rho,u) (Eq.25 :225 with Eq.20 :160, R9); step counter := 0.
+ * rho_dev = u_dev = NULL -> rho0, u = 0; else device arrays rho[N], u[3][N] of `real`.
+ * ESTATE without a workspace. */
+int rflbm_init(rflbm_t* h, const void* rho_dev, const void* u_dev);
+
+/* Advance nsteps time steps of Eq.24 (:221): one fused pull-stream + collide kernel launch per step
+ * (Eq.7 :87 pull form; Eq.2-3 :56-58; Eq.19 :153; Eq.20 :160; Eq.8-9 :93-99; Eq.10 :105).
+ * rflbm_step(a); rflbm_step(b) is bit-identical to rflbm_step(a+b).  ESTATE before init. */
+int rflbm_step(rflbm_t* h, int nsteps);
+
+/* rho[N], u[3][N] (device, `real`) of the current state: Eq.2-3, u = (j + F/2)/rho.  Solid nodes: 0. */
+int rflbm_moments(rflbm_t* h, void* rho_dev, void* u_dev);
+
+/* Synchronises the stream.  out_host = { sum rho, sum rho u_x,y,z, mean u_x,y,z, var u_x,y,z } over fluid sites
+ * (warp-shuffle + block reduction, fp64 accumulation). */
+int rflbm_diagnostics(rflbm_t* h, double out_host[10]);
+
+/* Canonical pre-collision populations f[27][N] (`real`, device) out of / into the handle.
+ * set also sets the step counter (checkpoint/resume: the RNG is counter based, so resuming is bit exact). */
+int rflbm_get_populations(rflbm_t* h, void* f_dev);
+int rflbm_set_populations(rflbm_t* h, const void* f_dev, uint64_t step);
+
+/* Test hook: what the step kernel draws at time `step` (R8): words[24][N] uint32 (6 Philox4x32-10 calls per
+ * site, word 4q+m = output m of call q) and normals[23][N] `real` (modes k = 4..26).  Either may be NULL. */
+int rflbm_debug_rng(rflbm_t* h, uint64_t step, void* words_dev, void* normals_dev);
+
+/* End-to-end job with HOST buffers (what bench.py's "e2e" times): copy rho_host[N], u_host[3][N] (`real`,
+ * ideally pinned) to the device scratch, init, advance nsteps, compute moments, copy them back to
+ * rho_out_host / u_out_host and synchronise.  scratch_dev: caller-owned device buffer of at least
+ * 4*N*sizeof(real) bytes.  rho_host = u_host = NULL -> uniform rho0, u=0 start (no upload). */
+int rflbm_run_host(rflbm_t* h, const void* rho_host, const void* u_host, int nsteps, void* rho_out_host,
+                   void* u_out_host, void* scratch_dev, size_t scratch_bytes);
+
+/* Number of kernels the handle has launched so far (bench.py's gpu_launches). */
+uint64_t rflbm_launch_count(const rflbm_t* h);
+
+uint64_t rflbm_step_count(const rflbm_t* h);
+const char* rflbm_last_error(const rflbm_t* h);
+
+/* Frees the host handle only (the workspace belongs to the caller). */
+int rflbm_destroy(rflbm_t* h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RFLBM_H */

@@ -1,0 +1,185 @@
+"""Thin ctypes binding of the C-ABI library (include/rflbm.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of csrc/; PyTorch is used for device memory and
+streams (the library itself never allocates device memory).  There is NO CPU fallback: if
+csrc/librflbm.so is missing or CUDA is unavailable, construction raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+F64, F32 = 0, 1
+OK, EINVAL, ESTATE, ENOMEM, ECUDA = 0, -1, -2, -3, -4
+Q = 27
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "csrc", "librflbm.so")
+_lib = None
+
+# every symbol include/rflbm.h declares: name -> (restype, argtypes)
+_vp, _u64, _i32, _dbl, _sz = C.c_void_p, C.c_uint64, C.c_int, C.c_double, C.c_size_t
+SYMBOLS = {
+    "rflbm_create": (_i32, [_i32, _i32, _i32, _dbl, _dbl, _dbl, _u64, _i32, C.POINTER(_vp)]),
+    "rflbm_workspace_bytes": (_sz, [_vp]),
+    "rflbm_set_workspace": (_i32, [_vp, _vp, _sz]),
+    "rflbm_set_stream": (_i32, [_vp, _vp]),
+    "rflbm_set_walls_z": (_i32, [_vp, _i32]),
+    "rflbm_set_force": (_i32, [_vp, _dbl, _dbl, _dbl]),
+    "rflbm_init": (_i32, [_vp, _vp, _vp]),
+    "rflbm_step": (_i32, [_vp, _i32]),
+    "rflbm_moments": (_i32, [_vp, _vp, _vp]),
+    "rflbm_diagnostics": (_i32, [_vp, C.POINTER(_dbl)]),
+    "rflbm_get_populations": (_i32, [_vp, _vp]),
+    "rflbm_set_populations": (_i32, [_vp, _vp, _u64]),
+    "rflbm_debug_rng": (_i32, [_vp, _u64, _vp, _vp]),
+    "rflbm_run_host": (_i32, [_vp, _vp, _vp, _i32, _vp, _vp, _vp, _sz]),
+    "rflbm_launch_count": (_u64, [_vp]),
+    "rflbm_step_count": (_u64, [_vp]),
+    "rflbm_last_error": (C.c_char_p, [_vp]),
+    "rflbm_destroy": (_i32, [_vp]),
+}
+
+
+class RflbmError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"rflbm error {code}: {msg}")
+        self.code = code
+
+
+def load():
+    """dlopen csrc/librflbm.so (built by paper_2507_08820_b200.build); fails loudly if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} is missing: run `python -m paper_2507_08820_b200.build` "
+                           "(there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    for name, (res, args) in SYMBOLS.items():
+        fn = getattr(lib, name)
+        fn.restype = res
+        fn.argtypes = args
+    _lib = lib
+    return lib
+
+
+def _ptr(t):
+    return 0 if t is None else t.data_ptr()
+
+
+class Rflbm:
+    """One simulation handle.  Tensors are torch CUDA tensors in the x-fastest layout
+    rho[nz,ny,nx], u[3,nz,ny,nx], f[27,nz,ny,nx] (canonical velocity order), dtype float64 or float32."""
+
+    def __init__(self, nx, ny, nz, tau, kT, rho0=1.0, seed=0, precision=F64, device="cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("CUDA is not available: the rflbm path has no CPU fallback")
+        self.torch = torch
+        self.lib = load()
+        self.nx, self.ny, self.nz = nx, ny, nz
+        self.shape = (nz, ny, nx)
+        self.n = nx * ny * nz
+        self.precision = precision
+        self.dtype = torch.float64 if precision == F64 else torch.float32
+        self.device = torch.device(device)
+        h = _vp()
+        rc = self.lib.rflbm_create(nx, ny, nz, tau, kT, rho0, seed, precision, C.byref(h))
+        if rc != OK:
+            raise RflbmError(rc, "rflbm_create: invalid argument")
+        self.h = h
+        nbytes = self.lib.rflbm_workspace_bytes(self.h)
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)   # owned here, borrowed by C
+            self._ck(self.lib.rflbm_set_workspace(self.h, self.workspace.data_ptr(), nbytes))
+            st = stream if stream is not None else torch.cuda.current_stream(self.device)
+            self.stream = st
+            self._ck(self.lib.rflbm_set_stream(self.h, st.cuda_stream))
+
+    def _ck(self, rc):
+        if rc != OK:
+            raise RflbmError(rc, self.lib.rflbm_last_error(self.h).decode())
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.lib.rflbm_destroy(self.h)
+            self.h = None
+            self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_walls_z(self, on=True):
+        self._ck(self.lib.rflbm_set_walls_z(self.h, int(on)))
+
+    def set_force(self, gx, gy, gz):
+        self._ck(self.lib.rflbm_set_force(self.h, gx, gy, gz))
+
+    def _field(self, t, lead=()):
+        t = t.to(device=self.device, dtype=self.dtype).contiguous()
+        assert tuple(t.shape) == tuple(lead) + self.shape, (t.shape, lead, self.shape)
+        return t
+
+    def init(self, rho=None, u=None):
+        if rho is None:
+            self._ck(self.lib.rflbm_init(self.h, None, None))
+        else:
+            rho, u = self._field(rho), self._field(u, (3,))
+            self._ck(self.lib.rflbm_init(self.h, rho.data_ptr(), u.data_ptr()))
+            self._keep = (rho, u)     # alive until the stream has consumed them
+
+    def step(self, n=1):
+        self._ck(self.lib.rflbm_step(self.h, int(n)))
+
+    def moments(self, rho=None, u=None):
+        t = self.torch
+        if rho is None:
+            rho = t.empty(self.shape, dtype=self.dtype, device=self.device)
+            u = t.empty((3,) + self.shape, dtype=self.dtype, device=self.device)
+        self._ck(self.lib.rflbm_moments(self.h, rho.data_ptr(), u.data_ptr()))
+        return rho, u
+
+    def diagnostics(self):
+        out = (_dbl * 10)()
+        self._ck(self.lib.rflbm_diagnostics(self.h, out))
+        return list(out)
+
+    def get_populations(self, f=None):
+        if f is None:
+            f = self.torch.empty((Q,) + self.shape, dtype=self.dtype, device=self.device)
+        self._ck(self.lib.rflbm_get_populations(self.h, f.data_ptr()))
+        return f
+
+    def set_populations(self, f, step=0):
+        f = self._field(f, (Q,))
+        self._ck(self.lib.rflbm_set_populations(self.h, f.data_ptr(), int(step)))
+        self._keep = (f,)
+
+    def debug_rng(self, step):
+        t = self.torch
+        words = t.empty((24,) + self.shape, dtype=t.int32, device=self.device)
+        normals = t.empty((23,) + self.shape, dtype=self.dtype, device=self.device)
+        self._ck(self.lib.rflbm_debug_rng(self.h, int(step), words.data_ptr(), normals.data_ptr()))
+        return words, normals
+
+    def run_host(self, rho_host, u_host, nsteps, rho_out_host, u_out_host, scratch=None):
+        """End-to-end job on HOST tensors (pinned for speed): upload, init, step, moments, download, sync."""
+        t = self.torch
+        es = 8 if self.precision == F64 else 4
+        if scratch is None:
+            scratch = t.empty(4 * self.n * es, dtype=t.uint8, device=self.device)
+        self._ck(self.lib.rflbm_run_host(self.h, _ptr(rho_host), _ptr(u_host), int(nsteps), rho_out_host.data_ptr(),
+                                         u_out_host.data_ptr(), scratch.data_ptr(), scratch.numel()))
+        return rho_out_host, u_out_host
+
+    @property
+    def step_count(self):
+        return int(self.lib.rflbm_step_count(self.h))
+
+    @property
+    def launch_count(self):
+        return int(self.lib.rflbm_launch_count(self.h))

@@ -1,0 +1,402 @@
+// rflbm.cu — C-ABI library (include/rflbm.h) over the kernels in rflbm_kernels.cuh.
+//
+// Host side only: argument validation, parameter marshalling, launches on the caller's stream.
+// The library never allocates device memory and never creates a stream (include/rflbm.h).
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "../../include/rflbm.h"
+#include "rflbm_kernels.cuh"
+
+using namespace rflbm_dev;
+
+struct rflbm {
+    int nx, ny, nz;
+    long long N;
+    double tau, kT, rho0;
+    uint64_t seed;
+    int precision;
+    int walls;
+    double g[3];
+    bool force;
+    void* ws;            // borrowed workspace
+    size_t ws_bytes;
+    void* buf[2];        // A-B population buffers inside ws
+    double* acc;         // 4 KiB reduction scratch inside ws
+    f64x2* tables;       // 8 KiB Box-Muller tables inside ws (uploaded by set_workspace)
+    int cur;             // buffer holding P_{t-1}
+    bool inited;
+    uint64_t t;
+    uint64_t launches;
+    cudaStream_t stream;
+    dim3 block, grid;
+    char err[512];
+};
+
+static size_t real_size(const rflbm* h) { return h->precision == RFLBM_F64 ? sizeof(double) : sizeof(float); }
+static size_t pop_bytes(const rflbm* h) { return (size_t)Q * (size_t)h->N * real_size(h); }
+static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+static constexpr size_t TABLE_BYTES = (LOG_TABLE_N + SC_TABLE_N) * sizeof(f64x2);
+
+static int fail(rflbm* h, int code, const char* fmt, ...)
+{
+    if (h) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(h->err, sizeof(h->err), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+static int check_cuda(rflbm* h, cudaError_t e, const char* what)
+{
+    if (e == cudaSuccess) return RFLBM_OK;
+    return fail(h, RFLBM_ECUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+static int after_launch(rflbm* h, const char* what)
+{
+    h->launches++;
+    return check_cuda(h, cudaPeekAtLastError(), what);
+}
+
+extern "C" int rflbm_create(int nx, int ny, int nz, double tau, double kT, double rho0, uint64_t seed, int precision,
+                            rflbm_t** out)
+{
+    if (!out) return RFLBM_EINVAL;
+    *out = nullptr;
+    if (nx < 1 || ny < 1 || nz < 1) return RFLBM_EINVAL;
+    if ((double)nx * (double)ny * (double)nz >= 4294967296.0) return RFLBM_EINVAL;
+    if (ny > 65535 * 16 || nz > 65535) return RFLBM_EINVAL;
+    if (!std::isfinite(tau) || !(tau > 0.5)) return RFLBM_EINVAL;
+    if (!std::isfinite(kT) || kT < 0.0) return RFLBM_EINVAL;
+    if (!std::isfinite(rho0) || !(rho0 > 0.0)) return RFLBM_EINVAL;
+    if (precision != RFLBM_F64 && precision != RFLBM_F32) return RFLBM_EINVAL;
+    rflbm* h = new (std::nothrow) rflbm;
+    if (!h) return RFLBM_ENOMEM;
+    memset(h, 0, sizeof(*h));
+    h->nx = nx; h->ny = ny; h->nz = nz;
+    h->N = (long long)nx * ny * nz;
+    h->tau = tau; h->kT = kT; h->rho0 = rho0; h->seed = seed; h->precision = precision;
+    // one thread per site; a warp covers 32 consecutive x whenever nx >= 32
+    int bx = 8;
+    while (bx < nx && bx < 128) bx *= 2;
+    const int by = 128 / bx;
+    h->block = dim3(bx, by, 1);
+    h->grid = dim3((nx + bx - 1) / bx, (ny + by - 1) / by, nz);
+    *out = h;
+    return RFLBM_OK;
+}
+
+extern "C" size_t rflbm_workspace_bytes(const rflbm_t* h)
+{
+    if (!h) return 0;
+    return 2 * align_up(pop_bytes(h), 256) + 4096 + TABLE_BYTES;
+}
+
+extern "C" int rflbm_set_workspace(rflbm_t* h, void* dev_ptr, size_t bytes)
+{
+    if (!h) return RFLBM_EINVAL;
+    if (!dev_ptr) return fail(h, RFLBM_EINVAL, "workspace pointer is NULL");
+    if (bytes < rflbm_workspace_bytes(h))
+        return fail(h, RFLBM_ENOMEM, "workspace too small: %zu < %zu bytes", bytes, rflbm_workspace_bytes(h));
+    if (((uintptr_t)dev_ptr & 255u) != 0) return fail(h, RFLBM_ENOMEM, "workspace must be 256-byte aligned");
+    h->ws = dev_ptr;
+    h->ws_bytes = bytes;
+    const size_t pb = align_up(pop_bytes(h), 256);
+    h->buf[0] = dev_ptr;
+    h->buf[1] = (char*)dev_ptr + pb;
+    h->acc = (double*)((char*)dev_ptr + 2 * pb);
+    h->tables = (f64x2*)((char*)dev_ptr + 2 * pb + 4096);
+    h->cur = 0;
+    h->inited = false;
+    // the only device write outside the stream: upload the Box-Muller tables (host-generated, long double libm)
+    static f64x2 host_tab[LOG_TABLE_N + SC_TABLE_N];
+    fill_normal_tables(host_tab, host_tab + LOG_TABLE_N);
+    return check_cuda(h, cudaMemcpy(h->tables, host_tab, TABLE_BYTES, cudaMemcpyHostToDevice), "table upload");
+}
+
+extern "C" int rflbm_set_stream(rflbm_t* h, void* cuda_stream)
+{
+    if (!h) return RFLBM_EINVAL;
+    h->stream = (cudaStream_t)cuda_stream;
+    return RFLBM_OK;
+}
+
+extern "C" int rflbm_set_walls_z(rflbm_t* h, int on)
+{
+    if (!h) return RFLBM_EINVAL;
+    if (on && h->nz < 3) return fail(h, RFLBM_EINVAL, "walls need nz >= 3");
+    if (h->inited) return fail(h, RFLBM_ESTATE, "set_walls_z must precede init/set_populations");
+    h->walls = on ? 1 : 0;
+    return RFLBM_OK;
+}
+
+extern "C" int rflbm_set_force(rflbm_t* h, double gx, double gy, double gz)
+{
+    if (!h) return RFLBM_EINVAL;
+    if (!std::isfinite(gx) || !std::isfinite(gy) || !std::isfinite(gz)) return fail(h, RFLBM_EINVAL, "non-finite force");
+    h->g[0] = gx; h->g[1] = gy; h->g[2] = gz;
+    h->force = (gx != 0.0 || gy != 0.0 || gz != 0.0);
+    return RFLBM_OK;
+}
+
+template <typename real>
+static FieldParams<real> field_params(const rflbm* h)
+{
+    FieldParams<real> P;
+    P.nx = h->nx; P.ny = h->ny; P.nz = h->nz; P.N = h->N;
+    P.hgx = (real)(0.5 * h->g[0]); P.hgy = (real)(0.5 * h->g[1]); P.hgz = (real)(0.5 * h->g[2]);
+    P.walls = h->walls;
+    return P;
+}
+
+template <typename real>
+static StepParams<real> step_params(const rflbm* h, uint64_t t)
+{
+    StepParams<real> P;
+    const double omega = 1.0 / h->tau;
+    P.nx = h->nx; P.ny = h->ny; P.nz = h->nz; P.N = h->N;
+    P.one_minus_omega = (real)(1.0 - omega);
+    P.noise_ghost = (real)std::sqrt(3.0 * h->kT);
+    P.noise_hydro = (real)std::sqrt(3.0 * h->kT * omega * (2.0 - omega));
+    P.gx = (real)h->g[0]; P.gy = (real)h->g[1]; P.gz = (real)h->g[2];
+    P.force_stress = (real)(1.0 - 0.5 * omega);
+    P.t_hi = (uint32_t)(t >> 32);
+    P.t_lo = (uint32_t)(t & 0xFFFFFFFFu);
+    P.keys = make_philox_keys(h->seed);
+    P.tables = h->tables;
+    return P;
+}
+
+// ---------------------------------------------------------------- init / import / export
+template <typename real>
+static int do_init(rflbm* h, const void* rho, const void* u)
+{
+    const FieldParams<real> P = field_params<real>(h);
+    if (h->walls)
+        init_kernel<real, true><<<h->grid, h->block, 0, h->stream>>>((const real*)rho, (const real*)u, h->rho0,
+                                                                      (real*)h->buf[0], (real*)h->buf[1], P);
+    else
+        init_kernel<real, false><<<h->grid, h->block, 0, h->stream>>>((const real*)rho, (const real*)u, h->rho0,
+                                                                       (real*)h->buf[0], (real*)h->buf[1], P);
+    return after_launch(h, "init_kernel");
+}
+
+extern "C" int rflbm_init(rflbm_t* h, const void* rho_dev, const void* u_dev)
+{
+    if (!h) return RFLBM_EINVAL;
+    if (!h->ws) return fail(h, RFLBM_ESTATE, "rflbm_init before rflbm_set_workspace");
+    if ((rho_dev == nullptr) != (u_dev == nullptr)) return fail(h, RFLBM_EINVAL, "rho and u must both be given or both NULL");
+    const int rc = (h->precision == RFLBM_F64) ? do_init<double>(h, rho_dev, u_dev) : do_init<float>(h, rho_dev, u_dev);
+    if (rc != RFLBM_OK) return rc;
+    h->cur = 0;
+    h->t = 0;
+    h->inited = true;
+    return RFLBM_OK;
+}
+
+template <typename real>
+static int do_import(rflbm* h, const void* f)
+{
+    const FieldParams<real> P = field_params<real>(h);
+    if (h->walls)
+        import_kernel<real, true><<<h->grid, h->block, 0, h->stream>>>((const real*)f, (real*)h->buf[0], (real*)h->buf[1], P);
+    else
+        import_kernel<real, false><<<h->grid, h->block, 0, h->stream>>>((const real*)f, (real*)h->buf[0], (real*)h->buf[1], P);
+    return after_launch(h, "import_kernel");
+}
+
+extern "C" int rflbm_set_populations(rflbm_t* h, const void* f_dev, uint64_t step)
+{
+    if (!h) return RFLBM_EINVAL;
+    if (!f_dev) return fail(h, RFLBM_EINVAL, "f_dev is NULL");
+    if (!h->ws) return fail(h, RFLBM_ESTATE, "rflbm_set_populations before rflbm_set_workspace");
+    const int rc = (h->precision == RFLBM_F64) ? do_import<double>(h, f_dev) : do_import<float>(h, f_dev);
+    if (rc != RFLBM_OK) return rc;
+    h->cur = 0;
+    h->t = step;
+    h->inited = true;
+    return RFLBM_OK;
+}
+
+template <typename real>
+static int do_export(rflbm* h, void* f)
+{
+    const FieldParams<real> P = field_params<real>(h);
+    if (h->walls)
+        export_kernel<real, true><<<h->grid, h->block, 0, h->stream>>>((const real*)h->buf[h->cur], (real*)f, P);
+    else
+        export_kernel<real, false><<<h->grid, h->block, 0, h->stream>>>((const real*)h->buf[h->cur], (real*)f, P);
+    return after_launch(h, "export_kernel");
+}
+
+extern "C" int rflbm_get_populations(rflbm_t* h, void* f_dev)
+{
+    if (!h) return RFLBM_EINVAL;
+    if (!f_dev) return fail(h, RFLBM_EINVAL, "f_dev is NULL");
+    if (!h->inited) return fail(h, RFLBM_ESTATE, "rflbm_get_populations before init");
+    return (h->precision == RFLBM_F64) ? do_export<double>(h, f_dev) : do_export<float>(h, f_dev);
+}
+
+// ---------------------------------------------------------------- the time step
+template <typename real, bool WALLS, bool FORCE, bool NOISE>
+static void launch_step(rflbm* h, const StepParams<real>& P)
+{
+    step_kernel<real, WALLS, FORCE, NOISE>
+        <<<h->grid, h->block, 0, h->stream>>>((const real*)h->buf[h->cur], (real*)h->buf[h->cur ^ 1], P);
+}
+
+template <typename real>
+static int do_step(rflbm* h, int nsteps)
+{
+    const bool noise = h->kT > 0.0;       // kT = 0: deterministic Reg-LBM, RNG skipped entirely (R17)
+    for (int s = 0; s < nsteps; ++s) {
+        const StepParams<real> P = step_params<real>(h, h->t);
+        const int variant = (h->walls ? 4 : 0) | (h->force ? 2 : 0) | (noise ? 1 : 0);
+        switch (variant) {
+            case 0: launch_step<real, false, false, false>(h, P); break;
+            case 1: launch_step<real, false, false, true>(h, P); break;
+            case 2: launch_step<real, false, true, false>(h, P); break;
+            case 3: launch_step<real, false, true, true>(h, P); break;
+            case 4: launch_step<real, true, false, false>(h, P); break;
+            case 5: launch_step<real, true, false, true>(h, P); break;
+            case 6: launch_step<real, true, true, false>(h, P); break;
+            default: launch_step<real, true, true, true>(h, P); break;
+        }
+        const int rc = after_launch(h, "step_kernel");
+        if (rc != RFLBM_OK) return rc;
+        h->cur ^= 1;
+        h->t += 1;
+    }
+    return RFLBM_OK;
+}
+
+extern "C" int rflbm_step(rflbm_t* h, int nsteps)
+{
+    if (!h) return RFLBM_EINVAL;
+    if (nsteps < 0) return fail(h, RFLBM_EINVAL, "nsteps < 0");
+    if (!h->inited) return fail(h, RFLBM_ESTATE, "rflbm_step before init");
+    return (h->precision == RFLBM_F64) ? do_step<double>(h, nsteps) : do_step<float>(h, nsteps);
+}
+
+// ---------------------------------------------------------------- observables
+template <typename real>
+static int do_moments(rflbm* h, void* rho, void* u)
+{
+    const FieldParams<real> P = field_params<real>(h);
+    if (h->walls)
+        moments_kernel<real, true><<<h->grid, h->block, 0, h->stream>>>((const real*)h->buf[h->cur], (real*)rho, (real*)u, P);
+    else
+        moments_kernel<real, false><<<h->grid, h->block, 0, h->stream>>>((const real*)h->buf[h->cur], (real*)rho, (real*)u, P);
+    return after_launch(h, "moments_kernel");
+}
+
+extern "C" int rflbm_moments(rflbm_t* h, void* rho_dev, void* u_dev)
+{
+    if (!h) return RFLBM_EINVAL;
+    if (!rho_dev || !u_dev) return fail(h, RFLBM_EINVAL, "rho_dev / u_dev is NULL");
+    if (!h->inited) return fail(h, RFLBM_ESTATE, "rflbm_moments before init");
+    return (h->precision == RFLBM_F64) ? do_moments<double>(h, rho_dev, u_dev) : do_moments<float>(h, rho_dev, u_dev);
+}
+
+template <typename real>
+static int do_diagnostics(rflbm* h)
+{
+    const FieldParams<real> P = field_params<real>(h);
+    if (h->walls)
+        diagnostics_kernel<real, true><<<h->grid, h->block, 0, h->stream>>>((const real*)h->buf[h->cur], h->acc, P);
+    else
+        diagnostics_kernel<real, false><<<h->grid, h->block, 0, h->stream>>>((const real*)h->buf[h->cur], h->acc, P);
+    return after_launch(h, "diagnostics_kernel");
+}
+
+extern "C" int rflbm_diagnostics(rflbm_t* h, double out_host[10])
+{
+    if (!h) return RFLBM_EINVAL;
+    if (!out_host) return fail(h, RFLBM_EINVAL, "out_host is NULL");
+    if (!h->inited) return fail(h, RFLBM_ESTATE, "rflbm_diagnostics before init");
+    int rc = check_cuda(h, cudaMemsetAsync(h->acc, 0, 10 * sizeof(double), h->stream), "cudaMemsetAsync");
+    if (rc != RFLBM_OK) return rc;
+    rc = (h->precision == RFLBM_F64) ? do_diagnostics<double>(h) : do_diagnostics<float>(h);
+    if (rc != RFLBM_OK) return rc;
+    double s[10];
+    rc = check_cuda(h, cudaMemcpyAsync(s, h->acc, sizeof(s), cudaMemcpyDeviceToHost, h->stream), "cudaMemcpyAsync");
+    if (rc != RFLBM_OK) return rc;
+    rc = check_cuda(h, cudaStreamSynchronize(h->stream), "cudaStreamSynchronize");
+    if (rc != RFLBM_OK) return rc;
+    const double nf = (double)h->nx * h->ny * (h->walls ? h->nz - 2 : h->nz);
+    out_host[0] = s[0];
+    for (int a = 0; a < 3; ++a) {
+        out_host[1 + a] = s[1 + a];
+        out_host[4 + a] = s[4 + a] / nf;
+        out_host[7 + a] = s[7 + a] / nf - out_host[4 + a] * out_host[4 + a];
+    }
+    return RFLBM_OK;
+}
+
+extern "C" int rflbm_debug_rng(rflbm_t* h, uint64_t step, void* words_dev, void* normals_dev)
+{
+    if (!h) return RFLBM_EINVAL;
+    if (!h->ws) return fail(h, RFLBM_ESTATE, "rflbm_debug_rng before rflbm_set_workspace");
+    if (h->precision == RFLBM_F64) {
+        const StepParams<double> P = step_params<double>(h, step);
+        debug_rng_kernel<double><<<h->grid, h->block, 0, h->stream>>>((uint32_t*)words_dev, (double*)normals_dev, P);
+    } else {
+        const StepParams<float> P = step_params<float>(h, step);
+        debug_rng_kernel<float><<<h->grid, h->block, 0, h->stream>>>((uint32_t*)words_dev, (float*)normals_dev, P);
+    }
+    return after_launch(h, "debug_rng_kernel");
+}
+
+// ---------------------------------------------------------------- host-buffer job (bench.py "e2e")
+extern "C" int rflbm_run_host(rflbm_t* h, const void* rho_host, const void* u_host, int nsteps, void* rho_out_host,
+                              void* u_out_host, void* scratch_dev, size_t scratch_bytes)
+{
+    if (!h) return RFLBM_EINVAL;
+    if (!rho_out_host || !u_out_host || !scratch_dev) return fail(h, RFLBM_EINVAL, "NULL output or scratch pointer");
+    if ((rho_host == nullptr) != (u_host == nullptr))
+        return fail(h, RFLBM_EINVAL, "rho_host and u_host must both be given or both NULL");
+    const size_t fb = (size_t)h->N * real_size(h);
+    if (scratch_bytes < 4 * fb) return fail(h, RFLBM_ENOMEM, "scratch too small: %zu < %zu bytes", scratch_bytes, 4 * fb);
+    char* d_rho = (char*)scratch_dev;
+    char* d_u = d_rho + fb;
+    int rc;
+    if (rho_host) {
+        rc = check_cuda(h, cudaMemcpyAsync(d_rho, rho_host, fb, cudaMemcpyHostToDevice, h->stream), "H2D rho");
+        if (rc != RFLBM_OK) return rc;
+        rc = check_cuda(h, cudaMemcpyAsync(d_u, u_host, 3 * fb, cudaMemcpyHostToDevice, h->stream), "H2D u");
+        if (rc != RFLBM_OK) return rc;
+        rc = rflbm_init(h, d_rho, d_u);
+    } else {
+        rc = rflbm_init(h, nullptr, nullptr);
+    }
+    if (rc != RFLBM_OK) return rc;
+    rc = rflbm_step(h, nsteps);
+    if (rc != RFLBM_OK) return rc;
+    rc = rflbm_moments(h, d_rho, d_u);
+    if (rc != RFLBM_OK) return rc;
+    rc = check_cuda(h, cudaMemcpyAsync(rho_out_host, d_rho, fb, cudaMemcpyDeviceToHost, h->stream), "D2H rho");
+    if (rc != RFLBM_OK) return rc;
+    rc = check_cuda(h, cudaMemcpyAsync(u_out_host, d_u, 3 * fb, cudaMemcpyDeviceToHost, h->stream), "D2H u");
+    if (rc != RFLBM_OK) return rc;
+    return check_cuda(h, cudaStreamSynchronize(h->stream), "cudaStreamSynchronize");
+}
+
+// ---------------------------------------------------------------- misc
+extern "C" uint64_t rflbm_launch_count(const rflbm_t* h) { return h ? h->launches : 0; }
+extern "C" uint64_t rflbm_step_count(const rflbm_t* h) { return h ? h->t : 0; }
+extern "C" const char* rflbm_last_error(const rflbm_t* h) { return h ? h->err : "NULL handle"; }
+
+extern "C" int rflbm_destroy(rflbm_t* h)
+{
+    if (!h) return RFLBM_EINVAL;
+    delete h;
+    return RFLBM_OK;
+}

@@ -1,0 +1,281 @@
+// rflbm_kernels.cuh — CUDA kernels of the Reg-FLBM path (sm_100a).
+//
+// Storage: two SoA buffers P[q][z][y][x] of `real` in the lex order of
+// rflbm_lattice.cuh, holding POST-collision, UN-streamed populations (R10).  A step PULLS
+// S_t[q](x) = P_{t-1}[q](x - c_q)  (Eq.7 :87; bounce-back: P_{t-1}[26-q](x) when x - c_q is solid, R12),
+// collides in registers and stores P_t[q](x): 27 neighbour reads (coalesced, at most one element off
+// alignment) and 27 aligned coalesced writes per site, nothing else.
+#pragma once
+#include "rflbm_collide.cuh"
+
+namespace rflbm_dev {
+
+struct SiteIndex {
+    int x, y, z;
+    bool valid;
+    long long s;        // x + nx (y + ny z)
+};
+
+// one thread per site: blockDim = (bx, by), grid = (ceil(nx/bx), ceil(ny/by), nz)
+__device__ __forceinline__ SiteIndex my_site(int nx, int ny)
+{
+    SiteIndex i;
+    i.x = blockIdx.x * blockDim.x + threadIdx.x;
+    i.y = blockIdx.y * blockDim.y + threadIdx.y;
+    i.z = blockIdx.z;
+    i.valid = (i.x < nx) && (i.y < ny);
+    i.s = (long long)i.x + (long long)nx * ((long long)i.y + (long long)ny * (long long)i.z);
+    return i;
+}
+
+// Pull-gather of the 27 pre-collision populations of a site into g[cz+1][cy+1][cx+1].
+template <typename real, bool WALLS>
+__device__ __forceinline__ void gather(const real* __restrict__ src, long long N, int nx, int ny, int nz,
+                                       const SiteIndex& i, real (&g)[3][3][3])
+{
+    // neighbour coordinates x - cx etc. with periodic wrap; index a = cx+1 reads from xs[a]
+    const int xs[3] = {(i.x + 1 == nx) ? 0 : i.x + 1, i.x, (i.x == 0) ? nx - 1 : i.x - 1};
+    const int ys[3] = {(i.y + 1 == ny) ? 0 : i.y + 1, i.y, (i.y == 0) ? ny - 1 : i.y - 1};
+    const int zs[3] = {(i.z + 1 == nz) ? 0 : i.z + 1, i.z, (i.z == 0) ? nz - 1 : i.z - 1};
+    const long long nxy = (long long)nx * ny;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        // with walls the fluid layers are z = 1..nz-2; x - c_q is solid iff (cz=+1 and z==1) or (cz=-1 and z==nz-2)
+        const bool bounce = WALLS && ((c == 2 && i.z == 1) || (c == 0 && i.z == nz - 2));
+#pragma unroll
+        for (int b = 0; b < 3; ++b) {
+            const long long row = (long long)nx * ((long long)ys[b] + (long long)ny * (long long)zs[c]);
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                const int q = a + 3 * b + 9 * c;
+                const long long pull = (long long)q * N + row + xs[a];
+                const long long back = (long long)(26 - q) * N + i.s;
+                g[c][b][a] = __ldg(src + ((WALLS && bounce) ? back : pull));
+            }
+        }
+    }
+    (void)nxy;
+}
+
+// copy the Box-Muller tables (8 KB) from global memory (L2 resident) to shared memory; ends with a barrier
+__device__ __forceinline__ void stage_tables(const f64x2* __restrict__ tab, f64x2* s_tab)
+{
+    const int tid = threadIdx.y * blockDim.x + threadIdx.x, nt = blockDim.x * blockDim.y;
+    const double2* src = reinterpret_cast<const double2*>(tab);
+    double2* dst = reinterpret_cast<double2*>(s_tab);
+    for (int n = tid; n < LOG_TABLE_N + SC_TABLE_N; n += nt) dst[n] = __ldg(src + n);
+    __syncthreads();
+}
+
+// ---------------------------------------------------------------- the hot kernel: one time step
+template <typename real, bool WALLS, bool FORCE, bool NOISE>
+__global__ void __launch_bounds__(128)
+step_kernel(const real* __restrict__ src, real* __restrict__ dst, const __grid_constant__ StepParams<real> P)
+{
+    constexpr bool TABLES = NOISE && sizeof(real) == 8;
+    __shared__ f64x2 s_tab[TABLES ? LOG_TABLE_N + SC_TABLE_N : 1];
+    if (TABLES) stage_tables(P.tables, s_tab);
+    const SiteIndex i = my_site(P.nx, P.ny);
+    if (!i.valid) return;
+    if (WALLS && (i.z == 0 || i.z == P.nz - 1)) return;    // solid layers are never updated
+    real g[3][3][3];
+    gather<real, WALLS>(src, P.N, P.nx, P.ny, P.nz, i, g);
+    collide<real, FORCE, NOISE>(g, P, (uint32_t)i.s, s_tab, s_tab + LOG_TABLE_N);
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int b = 0; b < 3; ++b)
+#pragma unroll
+            for (int a = 0; a < 3; ++a) __stcs(dst + (long long)(a + 3 * b + 9 * c) * P.N + i.s, g[c][b][a]);
+}
+
+// ---------------------------------------------------------------- observables
+template <typename real>
+struct FieldParams {
+    int nx, ny, nz;
+    long long N;
+    real hgx, hgy, hgz;   // g/2: reported velocity u = j/rho + g/2 (R13)
+    int walls;
+};
+
+template <typename real, bool WALLS>
+__global__ void __launch_bounds__(128)
+moments_kernel(const real* __restrict__ src, real* __restrict__ rho, real* __restrict__ u, const FieldParams<real> P)
+{
+    const SiteIndex i = my_site(P.nx, P.ny);
+    if (!i.valid) return;
+    if (WALLS && (i.z == 0 || i.z == P.nz - 1)) {
+        rho[i.s] = real(0); u[i.s] = real(0); u[P.N + i.s] = real(0); u[2 * P.N + i.s] = real(0);
+        return;
+    }
+    real g[3][3][3];
+    gather<real, WALLS>(src, P.N, P.nx, P.ny, P.nz, i, g);
+    const Moments10<real> m = forward_moments(g);
+    const real inv = real(1.0) / m.rho;
+    rho[i.s] = m.rho;
+    u[i.s] = fma(m.jx, inv, P.hgx);
+    u[P.N + i.s] = fma(m.jy, inv, P.hgy);
+    u[2 * P.N + i.s] = fma(m.jz, inv, P.hgz);
+}
+
+// sums over fluid sites of { rho, rho u_x,y,z, u_x,y,z, u_x^2,y^2,z^2 } -> acc[10] (fp64 atomics)
+template <typename real, bool WALLS>
+__global__ void __launch_bounds__(128)
+diagnostics_kernel(const real* __restrict__ src, double* __restrict__ acc, const FieldParams<real> P)
+{
+    const SiteIndex i = my_site(P.nx, P.ny);
+    double v[10];
+#pragma unroll
+    for (int n = 0; n < 10; ++n) v[n] = 0.0;
+    const bool fluid = i.valid && !(WALLS && (i.z == 0 || i.z == P.nz - 1));
+    if (fluid) {
+        real g[3][3][3];
+        gather<real, WALLS>(src, P.N, P.nx, P.ny, P.nz, i, g);
+        const Moments10<real> m = forward_moments(g);
+        const double rho = (double)m.rho;
+        const double ux = (double)m.jx / rho + (double)P.hgx;
+        const double uy = (double)m.jy / rho + (double)P.hgy;
+        const double uz = (double)m.jz / rho + (double)P.hgz;
+        v[0] = rho; v[1] = rho * ux; v[2] = rho * uy; v[3] = rho * uz;
+        v[4] = ux; v[5] = uy; v[6] = uz; v[7] = ux * ux; v[8] = uy * uy; v[9] = uz * uz;
+    }
+    __shared__ double part[4][10];
+    const int tid = threadIdx.y * blockDim.x + threadIdx.x;
+    const int lane = tid & 31, warp = tid >> 5;
+#pragma unroll
+    for (int n = 0; n < 10; ++n) {
+        double s = v[n];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+        if (lane == 0) part[warp][n] = s;
+    }
+    __syncthreads();
+    const int nwarps = (blockDim.x * blockDim.y + 31) >> 5;
+    if (tid < 10) {
+        double s = 0.0;
+        for (int w = 0; w < nwarps; ++w) s += part[w][tid];
+        atomicAdd(acc + tid, s);
+    }
+}
+
+// ---------------------------------------------------------------- state import / export (R10)
+// out[canonical i][s] = S_t[i](s): the same gather as the step; solid nodes export their stored values.
+template <typename real, bool WALLS>
+__global__ void __launch_bounds__(128)
+export_kernel(const real* __restrict__ src, real* __restrict__ out, const FieldParams<real> P)
+{
+    const SiteIndex i = my_site(P.nx, P.ny);
+    if (!i.valid) return;
+    if (WALLS && (i.z == 0 || i.z == P.nz - 1)) {
+#pragma unroll
+        for (int n = 0; n < Q; ++n) out[(long long)n * P.N + i.s] = src[(long long)lex_of_canon(n) * P.N + i.s];
+        return;
+    }
+    real g[3][3][3];
+    gather<real, WALLS>(src, P.N, P.nx, P.ny, P.nz, i, g);
+#pragma unroll
+    for (int n = 0; n < Q; ++n)
+        out[(long long)n * P.N + i.s] = g[canon_cz(n) + 1][canon_cy(n) + 1][canon_cx(n) + 1];
+}
+
+// P[q](s) = S[q](s + c_q), or S[26-q](s) when s + c_q is solid; solid nodes store S[q](s) unchanged.
+// `in` is canonical; written to both A and B buffers so that the never-updated solid layers agree.
+template <typename real, bool WALLS>
+__global__ void __launch_bounds__(128)
+import_kernel(const real* __restrict__ in, real* __restrict__ bufA, real* __restrict__ bufB, const FieldParams<real> P)
+{
+    const SiteIndex i = my_site(P.nx, P.ny);
+    if (!i.valid) return;
+    const bool solid = WALLS && (i.z == 0 || i.z == P.nz - 1);
+#pragma unroll
+    for (int n = 0; n < Q; ++n) {
+        const int cx = canon_cx(n), cy = canon_cy(n), cz = canon_cz(n);
+        const int q = lex_of(cx, cy, cz);
+        long long from = (long long)n * P.N + i.s;
+        if (!solid) {
+            const int zd = i.z + cz;
+            if (WALLS && (zd == 0 || zd == P.nz - 1)) {
+                // s + c_q solid: this slot is pulled back by the site itself as direction opp(q)
+                const int nopp = canon_of_lex(26 - q);
+                from = (long long)nopp * P.N + i.s;
+            } else {
+                const int xd = (i.x + cx + P.nx) % P.nx, yd = (i.y + cy + P.ny) % P.ny, zw = (zd + P.nz) % P.nz;
+                from = (long long)n * P.N + (long long)xd + (long long)P.nx * ((long long)yd + (long long)P.ny * zw);
+            }
+        }
+        const real v = in[from];
+        bufA[(long long)q * P.N + i.s] = v;
+        bufB[(long long)q * P.N + i.s] = v;
+    }
+}
+
+// equilibrium f^(0)_q(rho,u) in the product form of Eq.25 with Eq.20 (w_i and the Hermite sum factorise):
+//   f0 = rho phi(cx,ux) phi(cy,uy) phi(cz,uz),  phi(0,u) = 2/3 - u^2,  phi(+-1,u) = 1/6 +- u/2 + u^2/2
+__device__ __forceinline__ double phi1d(int c, double u)
+{
+    return (c == 0) ? (2.0 / 3.0 - u * u) : (1.0 / 6.0 + 0.5 * (double)c * u + 0.5 * u * u);
+}
+
+// init (R9, R10): P_{-1}[q](s) = f0_q(rho,u)(s + c_q), or f0_{26-q}(rho,u)(s) when s + c_q is solid.
+// rho/u NULL -> uniform rho0, u = 0.
+template <typename real, bool WALLS>
+__global__ void __launch_bounds__(128)
+init_kernel(const real* __restrict__ rho, const real* __restrict__ u, double rho0, real* __restrict__ bufA,
+            real* __restrict__ bufB, const FieldParams<real> P)
+{
+    const SiteIndex i = my_site(P.nx, P.ny);
+    if (!i.valid) return;
+    const bool solid = WALLS && (i.z == 0 || i.z == P.nz - 1);
+#pragma unroll 1
+    for (int q = 0; q < Q; ++q) {
+        int cx = q % 3 - 1, cy = (q / 3) % 3 - 1, cz = q / 9 - 1;
+        long long s = i.s;
+        if (!solid) {
+            const int zd = i.z + cz;
+            if (WALLS && (zd == 0 || zd == P.nz - 1)) {
+                cx = -cx; cy = -cy; cz = -cz;              // f0 of the opposite direction at the site itself
+            } else {
+                const int xd = (i.x + cx + P.nx) % P.nx, yd = (i.y + cy + P.ny) % P.ny, zw = (zd + P.nz) % P.nz;
+                s = (long long)xd + (long long)P.nx * ((long long)yd + (long long)P.ny * zw);
+            }
+        }
+        double r = rho0, ux = 0.0, uy = 0.0, uz = 0.0;
+        if (rho != nullptr) {
+            r = (double)rho[s]; ux = (double)u[s]; uy = (double)u[P.N + s]; uz = (double)u[2 * P.N + s];
+        }
+        const real v = (real)(r * phi1d(cx, ux) * phi1d(cy, uy) * phi1d(cz, uz));
+        bufA[(long long)q * P.N + i.s] = v;
+        bufB[(long long)q * P.N + i.s] = v;
+    }
+}
+
+// test hook: the words and normals the step kernel draws at (t_hi,t_lo)
+template <typename real>
+__global__ void __launch_bounds__(128)
+debug_rng_kernel(uint32_t* __restrict__ words, real* __restrict__ normals, const __grid_constant__ StepParams<real> P)
+{
+    constexpr bool TABLES = sizeof(real) == 8;
+    __shared__ f64x2 s_tab[TABLES ? LOG_TABLE_N + SC_TABLE_N : 1];
+    if (TABLES) stage_tables(P.tables, s_tab);
+    const SiteIndex i = my_site(P.nx, P.ny);
+    if (!i.valid) return;
+#pragma unroll
+    for (int call = 0; call < 6; ++call) {
+        uint32_t w[4];
+        philox4x32_10((uint32_t)i.s, P.t_hi, P.t_lo, (uint32_t)call, P.keys, w);
+        if (words != nullptr)
+#pragma unroll
+            for (int mth = 0; mth < 4; ++mth) words[(long long)(4 * call + mth) * P.N + i.s] = w[mth];
+        if (normals != nullptr)
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                real z0, z1;
+                normal_pair(w[2 * h], w[2 * h + 1], s_tab, s_tab + LOG_TABLE_N, z0, z1);
+                const int k = 4 + 4 * call + 2 * h;
+                normals[(long long)(k - 4) * P.N + i.s] = z0;
+                if (k + 1 < Q) normals[(long long)(k + 1 - 4) * P.N + i.s] = z1;
+            }
+    }
+}
+
+}  // namespace rflbm_dev

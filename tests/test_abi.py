@@ -1,0 +1,76 @@
+"""CPU-side checks of the boundary: the C-ABI library loads without a GPU and exports every symbol that
+include/rflbm.h declares; host-only argument validation (no compute calls)."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+from paper_2507_08820_b200 import binding, build
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    build.build()
+    return binding.load()
+
+
+def declared_symbols():
+    src = open(os.path.join(ROOT, "include", "rflbm.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(rflbm_[a-z_0-9]+)\s*\(", src)))
+
+
+def test_header_symbols_all_exported_and_bound(lib):
+    names = declared_symbols()
+    assert len(names) >= 18
+    for n in names:
+        assert hasattr(lib, n), n
+    assert sorted(binding.SYMBOLS) == names
+
+
+def test_create_validation_and_workspace_size(lib):
+    h = C.c_void_p()
+    bad = [(0, 4, 4, 1.0, 0.0, 1.0), (4, 4, 4, 0.5, 0.0, 1.0), (4, 4, 4, float("nan"), 0.0, 1.0),
+           (4, 4, 4, 1.0, -1e-9, 1.0), (4, 4, 4, 1.0, 0.0, 0.0), (2048, 2048, 2048, 1.0, 0.0, 1.0)]
+    for nx, ny, nz, tau, kT, rho0 in bad:
+        assert lib.rflbm_create(nx, ny, nz, tau, kT, rho0, 0, binding.F64, C.byref(h)) == binding.EINVAL
+    assert lib.rflbm_create(4, 4, 4, 1.0, 0.0, 1.0, 0, 5, C.byref(h)) == binding.EINVAL
+    assert lib.rflbm_create(4, 4, 4, 1.0, 0.0, 1.0, 0, binding.F64, None) == binding.EINVAL
+    assert lib.rflbm_create(16, 16, 16, 1.0, 1e-4, 1.0, 42, binding.F64, C.byref(h)) == binding.OK
+    assert lib.rflbm_workspace_bytes(h) == 2 * 27 * 4096 * 8 + 4096 + 8192
+    # state machine, host side only
+    assert lib.rflbm_step(h, 1) == binding.ESTATE
+    assert b"before init" in lib.rflbm_last_error(h)
+    assert lib.rflbm_init(h, None, None) == binding.ESTATE
+    assert lib.rflbm_set_workspace(h, 0x1000, 16) == binding.ENOMEM
+    assert lib.rflbm_set_workspace(h, 0x1001, 1 << 30) == binding.ENOMEM      # misaligned
+    assert lib.rflbm_set_force(h, float("inf"), 0.0, 0.0) == binding.EINVAL
+    assert lib.rflbm_step_count(h) == 0 and lib.rflbm_launch_count(h) == 0
+    assert lib.rflbm_destroy(h) == binding.OK
+    h32 = C.c_void_p()
+    assert lib.rflbm_create(4, 4, 2, 1.0, 0.0, 1.0, 0, binding.F32, C.byref(h32)) == binding.OK
+    assert lib.rflbm_workspace_bytes(h32) == 2 * 3584 + 4096 + 8192                  # 27*32*4 = 3456 -> 256-aligned 3584
+    assert lib.rflbm_set_walls_z(h32, 1) == binding.EINVAL                     # nz < 3
+    lib.rflbm_destroy(h32)
+
+
+def test_binding_fails_loudly_without_cuda():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    with pytest.raises(RuntimeError, match="no CPU fallback"):
+        binding.Rflbm(4, 4, 4, 1.0, 0.0)
+
+
+def test_product_never_imports_oracle():
+    """The product path must not route through the oracle (or read _work/)."""
+    pkg = os.path.join(ROOT, "paper_2507_08820_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                s = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle\b", s, flags=re.M), f
+                assert "rflbm_ref" not in s and "_work/" not in s, f

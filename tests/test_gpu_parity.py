@@ -1,0 +1,191 @@
+"""GPU parity: the CUDA path through the C-ABI against the CPU oracle, element by element on identical
+seeded inputs (configs[0] of BASELINE.json and ragged / walled / forced / fp32 variants)."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2507_08820_b200 import binding, synthetic
+
+pytestmark = pytest.mark.gpu
+
+TOL64 = 1e-11   # north_star: fp64 populations within 1e-11 max-abs after 100 steps
+TOL32 = 1e-5    # north_star: fp32 storage within 1e-5
+NT = min(8, oracle.max_threads())
+
+
+def torch_():
+    import torch
+    return torch
+
+
+def make_pair(nx, ny, nz, tau, kT, seed, precision=binding.F64, walls=False, force=None, rho0=1.0):
+    sim = binding.Rflbm(nx, ny, nz, tau, kT, rho0, seed, precision)
+    ref = oracle.Ref(nx, ny, nz, tau, kT, rho0, seed, precision, threads=NT)
+    if walls:
+        sim.set_walls_z(True); ref.set_walls_z(True)
+    if force is not None:
+        sim.set_force(*force); ref.set_force(*force)
+    return sim, ref
+
+
+def init_pair(sim, ref, fields=None):
+    torch = torch_()
+    if fields is None:
+        sim.init(); ref.init()
+    else:
+        rho, u = fields
+        sim.init(torch.from_numpy(rho), torch.from_numpy(u)); ref.init(rho, u)
+
+
+def pops(sim):
+    return sim.get_populations().cpu().numpy().astype(np.float64)
+
+
+def test_config1_rng_stream_bit_exact_and_normals():
+    sim, ref = make_pair(16, 16, 16, 1.0, 1e-4, 42)
+    for step in (0, 1, 99, 2 ** 32 + 5):
+        w_g, n_g = sim.debug_rng(step)
+        w_r, n_r = ref.debug_rng(step)
+        assert np.array_equal(w_g.cpu().numpy().view(np.uint32), w_r)          # bit exact
+        d = np.abs(n_g.cpu().numpy() - n_r)
+        assert d.max() < 2e-14, d.max()                                         # libm vs CUDA math: a few ulp of 6.8
+
+
+def test_config1_populations_100_steps():
+    sim, ref = make_pair(16, 16, 16, 1.0, 1e-4, 42)
+    init_pair(sim, ref)
+    assert np.abs(pops(sim) - ref.get_populations()).max() < 1e-16
+    for chunk in (1, 9, 90):
+        sim.step(chunk); ref.step(chunk)
+        err = np.abs(pops(sim) - ref.get_populations()).max()
+        assert err < TOL64, (sim.step_count, err)
+    assert sim.step_count == 100 == ref.step_count
+    # conservation and equipartition (config 1 checks)
+    d = sim.diagnostics()
+    n = 16 ** 3
+    assert abs(d[0] - n) < 1e-13 * n * 10
+    assert max(abs(v) for v in d[1:4]) / n < 1e-15
+    dr = ref.diagnostics()
+    assert np.abs(np.array(d) - dr).max() < 1e-9                              # mass sum of 4096 sites
+    rho, u = sim.moments()
+    u = u.cpu().numpy()
+    assert np.abs((u ** 2).mean(axis=(1, 2, 3)) / 1e-4 - 1.0).max() < 0.05
+    rr, ur = ref.moments()
+    assert np.abs(rho.cpu().numpy() - rr).max() < 1e-11 and np.abs(u - ur).max() < 1e-11
+
+
+@pytest.mark.parametrize("shape,tau,kT", [((5, 7, 9), 0.7, 1e-4), ((130, 6, 5), 0.51, 1e-4), ((40, 9, 4), 50.0, 1e-4),
+                                          ((1, 1, 1), 0.8, 1e-4), ((33, 33, 2), 0.9, 0.0), ((300, 3, 3), 1.5, 1e-3)])
+def test_ragged_shapes_smooth_init(shape, tau, kT):
+    """several blocks plus a ragged tail in x and y, non-trivial (rho,u) through rflbm_init"""
+    nx, ny, nz = shape
+    sim, ref = make_pair(nx, ny, nz, tau, kT, 7)
+    init_pair(sim, ref, synthetic.smooth_random_fields(nx, ny, nz, 5))
+    assert np.abs(pops(sim) - ref.get_populations()).max() < 1e-15
+    sim.step(30); ref.step(30)
+    assert np.abs(pops(sim) - ref.get_populations()).max() < TOL64
+
+
+def test_walls_and_force_fp64():
+    nx, ny, nz = 12, 10, 11
+    sim, ref = make_pair(nx, ny, nz, 0.9, 1e-4, 5, walls=True, force=(1e-5, -2e-6, 3e-6))
+    init_pair(sim, ref, synthetic.smooth_random_fields(nx, ny, nz, 9))
+    assert np.abs(pops(sim) - ref.get_populations()).max() < 1e-15
+    sim.step(60); ref.step(60)
+    assert np.abs(pops(sim) - ref.get_populations()).max() < TOL64
+    rho, u = sim.moments()
+    rr, ur = ref.moments()
+    assert np.abs(rho.cpu().numpy() - rr).max() < 1e-11 and np.abs(u.cpu().numpy() - ur).max() < 1e-11
+    assert (rho.cpu().numpy()[0] == 0).all() and (rho.cpu().numpy()[-1] == 0).all()
+    assert np.abs(np.array(sim.diagnostics()) - ref.diagnostics()).max() < 1e-10
+
+
+def test_walls_minimal_nz3_and_force_only_periodic():
+    sim, ref = make_pair(6, 5, 3, 0.8, 1e-4, 3, walls=True)
+    init_pair(sim, ref)
+    sim.step(20); ref.step(20)
+    assert np.abs(pops(sim) - ref.get_populations()).max() < TOL64
+    sim, ref = make_pair(6, 5, 4, 0.8, 0.0, 3, force=(1e-6, 0.0, -2e-6))
+    init_pair(sim, ref)
+    sim.step(10); ref.step(10)
+    assert np.abs(pops(sim) - ref.get_populations()).max() < 1e-14
+    d = sim.diagnostics()
+    assert abs(d[1] / (120 * 1e-6 * 10.5) - 1) < 1e-11                       # momentum grows by N rho0 g per step
+
+
+def test_fp32_channel_parity_100_steps():
+    """config 5 at test size: 16x16x18 channel, fp32 storage, walls, body force, 100 steps."""
+    nx, ny, nz = 16, 16, 18
+    sim, ref = make_pair(nx, ny, nz, 0.9, 1e-4, 5, precision=binding.F32, walls=True, force=(1e-6, 0.0, 0.0))
+    init_pair(sim, ref)
+    sim.step(100); ref.step(100)
+    err = np.abs(pops(sim) - ref.get_populations()).max()
+    assert err < TOL32, err
+    w_g, n_g = sim.debug_rng(17)
+    w_r, n_r = ref.debug_rng(17)
+    assert np.array_equal(w_g.cpu().numpy().view(np.uint32), w_r)
+    assert np.abs(n_g.cpu().numpy().astype(np.float64) - n_r).max() < 5e-4     # float Box-Muller, |r| up to 5.9
+
+
+def test_fp32_periodic_parity():
+    sim, ref = make_pair(20, 12, 7, 0.7, 1e-4, 8, precision=binding.F32)
+    init_pair(sim, ref, synthetic.smooth_random_fields(20, 12, 7, 2))
+    sim.step(100); ref.step(100)
+    assert np.abs(pops(sim) - ref.get_populations()).max() < TOL32
+
+
+def test_set_get_roundtrip_and_resume_bit_exact():
+    torch = torch_()
+    c, w = oracle.tables()[:2]
+    for walls in (False, True):
+        nx, ny, nz = 9, 6, 5
+        f = synthetic.random_population_field(nx, ny, nz, 4, w)
+        sim, ref = make_pair(nx, ny, nz, 0.8, 1e-4, 11, walls=walls)
+        sim.set_populations(torch.from_numpy(f), 17)
+        ref.set_populations(f, 17)
+        assert np.array_equal(pops(sim), f)                                    # import -> export is the identity
+        sim.step(25); ref.step(25)
+        assert sim.step_count == 42
+        assert np.abs(pops(sim) - ref.get_populations()).max() < TOL64
+    # step(50)+step(50) == step(100), and resume from an exported state, bit for bit
+    a = binding.Rflbm(16, 8, 8, 0.8, 1e-4, 1.0, 3); a.init(); a.step(100)
+    b = binding.Rflbm(16, 8, 8, 0.8, 1e-4, 1.0, 3); b.init(); b.step(50); b.step(50)
+    c2 = binding.Rflbm(16, 8, 8, 0.8, 1e-4, 1.0, 3); c2.set_populations(b.get_populations() * 0 + 1, 0)
+    c2.init(); c2.step(50)
+    d = binding.Rflbm(16, 8, 8, 0.8, 1e-4, 1.0, 3); d.set_populations(c2.get_populations(), c2.step_count); d.step(50)
+    fa = a.get_populations()
+    assert torch.equal(fa, b.get_populations()) and torch.equal(fa, d.get_populations())
+
+
+def test_kT0_equilibrium_fixed_point_and_error_codes():
+    torch = torch_()
+    sim = binding.Rflbm(8, 8, 8, 0.6, 0.0)
+    rho, u = synthetic.uniform_fields(8, 8, 8, 1.2, (0.05, -0.02, 0.08))
+    sim.init(torch.from_numpy(rho), torch.from_numpy(u))
+    f0 = sim.get_populations().clone()
+    sim.step(5)
+    assert (sim.get_populations() - f0).abs().max().item() < 1e-15
+    with pytest.raises(binding.RflbmError) as e:
+        sim.set_walls_z(True)                                                  # after init
+    assert e.value.code == binding.ESTATE
+    with pytest.raises(binding.RflbmError) as e:
+        sim.step(-1)
+    assert e.value.code == binding.EINVAL
+    fresh = binding.Rflbm(4, 4, 4, 1.0, 0.0)
+    with pytest.raises(binding.RflbmError) as e:
+        fresh.moments()
+    assert e.value.code == binding.ESTATE
+
+
+def test_run_host_matches_device_path():
+    torch = torch_()
+    nx, ny, nz = 24, 10, 6
+    rho, u = synthetic.smooth_random_fields(nx, ny, nz, 12)
+    sim, ref = make_pair(nx, ny, nz, 0.8, 1e-4, 21)
+    rho_h = torch.from_numpy(rho).pin_memory(); u_h = torch.from_numpy(u).pin_memory()
+    ro = torch.empty_like(rho_h).pin_memory(); uo = torch.empty_like(u_h).pin_memory()
+    sim.run_host(rho_h, u_h, 20, ro, uo)
+    ref.init(rho, u); ref.step(20)
+    rr, ur = ref.moments()
+    assert np.abs(ro.numpy() - rr).max() < 1e-11 and np.abs(uo.numpy() - ur).max() < 1e-11
+    assert sim.launch_count == 22                                             # init + 20 steps + moments
