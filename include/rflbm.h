@@ -72,6 +72,13 @@ int rflbm_init(rflbm_t* h, const void* rho_dev, const void* u_dev);
  * rflbm_step(a); rflbm_step(b) is bit-identical to rflbm_step(a+b).  ESTATE before init. */
 int rflbm_step(rflbm_t* h, int nsteps);
 
+/* Which implementation of the step kernel rflbm_step launches.  AUTO (default): the TMA-staged kernel when the
+ * lattice allows it (fp64, nx >= 128, nx even), else the plain one-thread-per-site kernel.  PLAIN forces the
+ * latter; TMA fails with EINVAL at rflbm_step if the lattice does not allow it.  All variants compute the same
+ * update (same results up to the bit: identical arithmetic, only the data movement differs). */
+enum { RFLBM_KERNEL_AUTO = 0, RFLBM_KERNEL_PLAIN = 1, RFLBM_KERNEL_TMA = 2 };
+int rflbm_set_kernel_variant(rflbm_t* h, int variant);
+
 /* rho[N], u[3][N] (device, `real`) of the current state: Eq.2-3, u = (j + F/2)/rho.  Solid nodes: 0. */
 int rflbm_moments(rflbm_t* h, void* rho_dev, void* u_dev);
 

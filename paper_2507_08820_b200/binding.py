@@ -11,6 +11,7 @@ import os
 
 F64, F32 = 0, 1
 OK, EINVAL, ESTATE, ENOMEM, ECUDA = 0, -1, -2, -3, -4
+KERNEL_AUTO, KERNEL_PLAIN, KERNEL_TMA = 0, 1, 2
 Q = 27
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -26,6 +27,7 @@ SYMBOLS = {
     "rflbm_set_stream": (_i32, [_vp, _vp]),
     "rflbm_set_walls_z": (_i32, [_vp, _i32]),
     "rflbm_set_force": (_i32, [_vp, _dbl, _dbl, _dbl]),
+    "rflbm_set_kernel_variant": (_i32, [_vp, _i32]),
     "rflbm_init": (_i32, [_vp, _vp, _vp]),
     "rflbm_step": (_i32, [_vp, _i32]),
     "rflbm_moments": (_i32, [_vp, _vp, _vp]),
@@ -115,6 +117,9 @@ class Rflbm:
 
     def set_walls_z(self, on=True):
         self._ck(self.lib.rflbm_set_walls_z(self.h, int(on)))
+
+    def set_kernel_variant(self, variant):
+        self._ck(self.lib.rflbm_set_kernel_variant(self.h, int(variant)))
 
     def set_force(self, gx, gy, gz):
         self._ck(self.lib.rflbm_set_force(self.h, gx, gy, gz))

@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(CSRC, "librflbm.so")
 SOURCES = ["rflbm.cu"]
-HEADERS = ["rflbm_lattice.cuh", "rflbm_fastmath.cuh", "rflbm_rng.cuh", "rflbm_collide.cuh", "rflbm_kernels.cuh",
+HEADERS = ["rflbm_lattice.cuh", "rflbm_fastmath.cuh", "rflbm_rng.cuh", "rflbm_collide.cuh", "rflbm_kernels.cuh", "rflbm_step_tma.cuh",
            os.path.join("..", "..", "include", "rflbm.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]

@@ -12,6 +12,7 @@
 
 #include "../../include/rflbm.h"
 #include "rflbm_kernels.cuh"
+#include "rflbm_step_tma.cuh"
 
 using namespace rflbm_dev;
 
@@ -35,6 +36,10 @@ struct rflbm {
     uint64_t launches;
     cudaStream_t stream;
     dim3 block, grid;
+    CUtensorMap tmap[2];  // TMA descriptors of the two population buffers (fp64, nx >= 128, nx even)
+    bool tma_ok;
+    int variant;          // RFLBM_KERNEL_AUTO / _PLAIN / _TMA
+    int rows_per_block;   // y rows walked by one block of the TMA kernel
     char err[512];
 };
 
@@ -66,6 +71,32 @@ static int after_launch(rflbm* h, const char* what)
     return check_cuda(h, cudaPeekAtLastError(), what);
 }
 
+// cuTensorMapEncodeTiled through the runtime's driver entry point: libcuda is not linked, so the library still
+// loads on a machine without a driver (the CPU-side ABI tests).
+typedef CUresult (*encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// 4-D view [27][nz][ny][nx] of one fp64 population buffer, box = BOX_X consecutive x of one row of one array
+static bool make_tensor_map(rflbm* h, void* base, CUtensorMap* out)
+{
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+        qres != cudaDriverEntryPointSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    const cuuint64_t dims[4] = {(cuuint64_t)h->nx, (cuuint64_t)h->ny, (cuuint64_t)h->nz, (cuuint64_t)Q};
+    const cuuint64_t strides[3] = {(cuuint64_t)h->nx * 8, (cuuint64_t)h->nx * h->ny * 8, (cuuint64_t)h->N * 8};
+    const cuuint32_t box[4] = {BOX_X, 1, 1, 1};   // 130 elements: 16-byte aligned starts, see rflbm_step_tma.cuh
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    const CUresult r = ((encode_tiled_fn)fn)(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box, estr,
+                                             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                             CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS;
+}
+
 extern "C" int rflbm_create(int nx, int ny, int nz, double tau, double kT, double rho0, uint64_t seed, int precision,
                             rflbm_t** out)
 {
@@ -90,6 +121,7 @@ extern "C" int rflbm_create(int nx, int ny, int nz, double tau, double kT, doubl
     const int by = 128 / bx;
     h->block = dim3(bx, by, 1);
     h->grid = dim3((nx + bx - 1) / bx, (ny + by - 1) / by, nz);
+    h->rows_per_block = 16;
     *out = h;
     return RFLBM_OK;
 }
@@ -119,7 +151,13 @@ extern "C" int rflbm_set_workspace(rflbm_t* h, void* dev_ptr, size_t bytes)
     // the only device write outside the stream: upload the Box-Muller tables (host-generated, long double libm)
     static f64x2 host_tab[LOG_TABLE_N + SC_TABLE_N];
     fill_normal_tables(host_tab, host_tab + LOG_TABLE_N);
-    return check_cuda(h, cudaMemcpy(h->tables, host_tab, TABLE_BYTES, cudaMemcpyHostToDevice), "table upload");
+    const int rc = check_cuda(h, cudaMemcpy(h->tables, host_tab, TABLE_BYTES, cudaMemcpyHostToDevice), "table upload");
+    if (rc != RFLBM_OK) return rc;
+    // TMA path: fp64, rows of at least one 128-site tile, row pitch a multiple of 16 bytes
+    h->tma_ok = false;
+    if (h->precision == RFLBM_F64 && h->nx >= TILE_X && h->nx % 2 == 0)
+        h->tma_ok = make_tensor_map(h, h->buf[0], &h->tmap[0]) && make_tensor_map(h, h->buf[1], &h->tmap[1]);
+    return RFLBM_OK;
 }
 
 extern "C" int rflbm_set_stream(rflbm_t* h, void* cuda_stream)
@@ -253,13 +291,50 @@ static void launch_step(rflbm* h, const StepParams<real>& P)
         <<<h->grid, h->block, 0, h->stream>>>((const real*)h->buf[h->cur], (real*)h->buf[h->cur ^ 1], P);
 }
 
+template <bool WALLS, bool FORCE, bool NOISE>
+static void launch_step_tma(rflbm* h, const StepParams<double>& P)
+{
+    const dim3 grid((h->nx + TILE_X - 1) / TILE_X, (h->ny + h->rows_per_block - 1) / h->rows_per_block, h->nz);
+    step_kernel_tma<WALLS, FORCE, NOISE><<<grid, TILE_X, 0, h->stream>>>(
+        h->tmap[h->cur], (const double*)h->buf[h->cur], (double*)h->buf[h->cur ^ 1], P, h->rows_per_block);
+}
+
+static bool use_tma(const rflbm* h) { return h->tma_ok && h->variant != RFLBM_KERNEL_PLAIN; }
+
+template <typename real>
+static void dispatch_tma(rflbm*, const StepParams<real>&, int) {}
+template <>
+void dispatch_tma<double>(rflbm* h, const StepParams<double>& P, int variant)
+{
+    switch (variant) {
+        case 0: launch_step_tma<false, false, false>(h, P); break;
+        case 1: launch_step_tma<false, false, true>(h, P); break;
+        case 2: launch_step_tma<false, true, false>(h, P); break;
+        case 3: launch_step_tma<false, true, true>(h, P); break;
+        case 4: launch_step_tma<true, false, false>(h, P); break;
+        case 5: launch_step_tma<true, false, true>(h, P); break;
+        case 6: launch_step_tma<true, true, false>(h, P); break;
+        default: launch_step_tma<true, true, true>(h, P); break;
+    }
+}
+
 template <typename real>
 static int do_step(rflbm* h, int nsteps)
 {
     const bool noise = h->kT > 0.0;       // kT = 0: deterministic Reg-LBM, RNG skipped entirely (R17)
+    if (h->variant == RFLBM_KERNEL_TMA && !h->tma_ok)
+        return fail(h, RFLBM_EINVAL, "TMA kernel needs fp64, nx >= 128 and nx even");
     for (int s = 0; s < nsteps; ++s) {
         const StepParams<real> P = step_params<real>(h, h->t);
         const int variant = (h->walls ? 4 : 0) | (h->force ? 2 : 0) | (noise ? 1 : 0);
+        if (use_tma(h)) {
+            dispatch_tma<real>(h, P, variant);
+            const int rc = after_launch(h, "step_kernel_tma");
+            if (rc != RFLBM_OK) return rc;
+            h->cur ^= 1;
+            h->t += 1;
+            continue;
+        }
         switch (variant) {
             case 0: launch_step<real, false, false, false>(h, P); break;
             case 1: launch_step<real, false, false, true>(h, P); break;
@@ -387,6 +462,15 @@ extern "C" int rflbm_run_host(rflbm_t* h, const void* rho_host, const void* u_ho
     rc = check_cuda(h, cudaMemcpyAsync(u_out_host, d_u, 3 * fb, cudaMemcpyDeviceToHost, h->stream), "D2H u");
     if (rc != RFLBM_OK) return rc;
     return check_cuda(h, cudaStreamSynchronize(h->stream), "cudaStreamSynchronize");
+}
+
+extern "C" int rflbm_set_kernel_variant(rflbm_t* h, int variant)
+{
+    if (!h) return RFLBM_EINVAL;
+    if (variant != RFLBM_KERNEL_AUTO && variant != RFLBM_KERNEL_PLAIN && variant != RFLBM_KERNEL_TMA)
+        return fail(h, RFLBM_EINVAL, "unknown kernel variant %d", variant);
+    h->variant = variant;
+    return RFLBM_OK;
 }
 
 // ---------------------------------------------------------------- misc

@@ -189,3 +189,33 @@ def test_run_host_matches_device_path():
     rr, ur = ref.moments()
     assert np.abs(ro.numpy() - rr).max() < 1e-11 and np.abs(uo.numpy() - ur).max() < 1e-11
     assert sim.launch_count == 22                                             # init + 20 steps + moments
+
+
+@pytest.mark.parametrize("shape,walls,force,kT", [((128, 4, 3), False, None, 1e-4), ((256, 5, 4), True, (1e-5, 2e-6, -3e-6), 1e-4),
+                                                 ((300, 3, 3), False, None, 1e-4), ((130, 18, 5), True, None, 0.0),
+                                                 ((384, 20, 2), False, (1e-6, 0.0, 0.0), 1e-3)])
+def test_tma_kernel_matches_plain_kernel_and_oracle(shape, walls, force, kT):
+    """The TMA-staged step kernel (fp64, nx >= 128, nx even) against the plain kernel (bit for bit: same
+    arithmetic) and the oracle; shapes span several x tiles, a ragged last tile, > rows_per_block rows, walls."""
+    torch = torch_()
+    nx, ny, nz = shape
+    fields = synthetic.smooth_random_fields(nx, ny, nz, 13)
+    outs = {}
+    for variant in (binding.KERNEL_TMA, binding.KERNEL_PLAIN):
+        sim, ref = make_pair(nx, ny, nz, 0.8, kT, 17, walls=walls, force=force)
+        sim.set_kernel_variant(variant)
+        init_pair(sim, ref, fields)
+        sim.step(12)
+        outs[variant] = sim.get_populations()
+    ref.step(12)
+    assert torch.equal(outs[binding.KERNEL_TMA], outs[binding.KERNEL_PLAIN])
+    assert np.abs(outs[binding.KERNEL_TMA].cpu().numpy() - ref.get_populations()).max() < TOL64
+
+
+def test_tma_variant_rejected_when_lattice_does_not_allow_it():
+    sim = binding.Rflbm(33, 4, 4, 0.8, 1e-4)
+    sim.set_kernel_variant(binding.KERNEL_TMA)
+    sim.init()
+    with pytest.raises(binding.RflbmError) as e:
+        sim.step(1)
+    assert e.value.code == binding.EINVAL
