@@ -46,6 +46,7 @@ def parse_args():
     p.add_argument("--size", type=int, default=WORKLOAD["size"])
     p.add_argument("--kT", type=float, default=WORKLOAD["kT"])
     p.add_argument("--precision", default="f64", choices=["f64", "f32"])
+    p.add_argument("--variant", default="auto", choices=["auto", "plain", "tma"])
     p.add_argument("--no-e2e", action="store_true")
     p.add_argument("--no-cpu", action="store_true")
     p.add_argument("--cpu-seconds", type=float, default=12.0)
@@ -223,6 +224,7 @@ def run_ours(args):
     K, W = args.steps, max(3, args.warmup)
 
     sim = binding.Rflbm(n, n, n, WORKLOAD["tau"], args.kT, WORKLOAD["rho0"], WORKLOAD["seed"], prec, device=dev)
+    sim.set_kernel_variant({"auto": binding.KERNEL_AUTO, "plain": binding.KERNEL_PLAIN, "tma": binding.KERNEL_TMA}[args.variant])
     sim.init()
     sim.step(W)                                     # warm-up: also thermalises the state
     torch.cuda.synchronize(dev)
