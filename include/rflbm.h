@@ -45,7 +45,7 @@ int rflbm_create(int nx, int ny, int nz, double tau, double kT, double rho0, uin
                  rflbm_t** out);
 
 /* Bytes of device workspace the handle needs: two population buffers 2*27*N*sizeof(real) (A-B scheme)
- * plus a 4 KiB reduction scratch and 8 KiB of Box-Muller tables (uploaded here, synchronously). */
+ * plus a 4 KiB reduction scratch and 12 KiB of Box-Muller tables (uploaded by rflbm_set_workspace, synchronously). */
 size_t rflbm_workspace_bytes(const rflbm_t* h);
 
 /* Borrow `bytes` of device memory at dev_ptr (256-byte aligned) as the workspace.
@@ -92,7 +92,9 @@ int rflbm_get_populations(rflbm_t* h, void* f_dev);
 int rflbm_set_populations(rflbm_t* h, const void* f_dev, uint64_t step);
 
 /* Test hook: what the step kernel draws at time `step` (R8): words[24][N] uint32 (6 Philox4x32-10 calls per
- * site, word 4q+m = output m of call q) and normals[23][N] `real` (modes k = 4..26).  Either may be NULL. */
+ * site, word 4q+m = output m of call q) and normals[23][N] `real` (modes k = 4..26).  Either may be NULL.
+ * Synchronises the stream; ECUDA if the step kernel's hand-scheduled Philox rounds (csrc/rflbm_rng.cuh) disagree
+ * with the plain ten-round loop at any site. */
 int rflbm_debug_rng(rflbm_t* h, uint64_t step, void* words_dev, void* normals_dev);
 
 /* End-to-end job with HOST buffers (what bench.py's "e2e" times): copy rho_host[N], u_host[3][N] (`real`,

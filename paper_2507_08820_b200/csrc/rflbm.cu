@@ -201,14 +201,21 @@ static StepParams<real> step_params(const rflbm* h, uint64_t t)
     StepParams<real> P;
     const double omega = 1.0 / h->tau;
     P.nx = h->nx; P.ny = h->ny; P.nz = h->nz; P.N = h->N;
-    P.one_minus_omega = (real)(1.0 - omega);
-    P.noise_ghost = (real)std::sqrt(3.0 * h->kT);
-    P.noise_hydro = (real)std::sqrt(3.0 * h->kT * omega * (2.0 - omega));
+    P.half_omc = (real)(0.5 * (1.0 - omega));
+    // Eq.9 per unit sqrt(rho): sqrt(3 kT omega_k (2 - omega_k)) prod_axis s_p, s = (1, sqrt3/6, sqrt2/6)
+    const double nh = std::sqrt(3.0 * h->kT * omega * (2.0 - omega)), ng = std::sqrt(3.0 * h->kT);
+    const double s1 = std::sqrt(3.0) / 6.0, s2 = std::sqrt(2.0) / 6.0;
+    P.amp[AMP_200] = (real)(nh * s2);
+    P.amp[AMP_110] = (real)(nh * s1 * s1);
+    P.amp[AMP_210] = (real)(ng * s2 * s1);
+    P.amp[AMP_111] = (real)(ng * s1 * s1 * s1);
+    P.amp[AMP_220] = (real)(ng * s2 * s2);
+    P.amp[AMP_211] = (real)(ng * s2 * s1 * s1);
+    P.amp[AMP_221] = (real)(ng * s2 * s2 * s1);
+    P.amp[AMP_222] = (real)(ng * s2 * s2 * s2);
     P.gx = (real)h->g[0]; P.gy = (real)h->g[1]; P.gz = (real)h->g[2];
     P.force_stress = (real)(1.0 - 0.5 * omega);
-    P.t_hi = (uint32_t)(t >> 32);
-    P.t_lo = (uint32_t)(t & 0xFFFFFFFFu);
-    P.keys = make_philox_keys(h->seed);
+    P.rng = make_philox_step(h->seed, t);
     P.tables = h->tables;
     return P;
 }
@@ -420,14 +427,29 @@ extern "C" int rflbm_debug_rng(rflbm_t* h, uint64_t step, void* words_dev, void*
 {
     if (!h) return RFLBM_EINVAL;
     if (!h->ws) return fail(h, RFLBM_ESTATE, "rflbm_debug_rng before rflbm_set_workspace");
+    // acc[16] counts the sites where the hand-scheduled Philox differs from the textbook loop
+    unsigned long long* mismatch = (unsigned long long*)(h->acc + 16);
+    int rc = check_cuda(h, cudaMemsetAsync(mismatch, 0, sizeof(*mismatch), h->stream), "cudaMemsetAsync");
+    if (rc != RFLBM_OK) return rc;
+    const uint32_t t_hi = (uint32_t)(step >> 32), t_lo = (uint32_t)(step & 0xFFFFFFFFu);
     if (h->precision == RFLBM_F64) {
         const StepParams<double> P = step_params<double>(h, step);
-        debug_rng_kernel<double><<<h->grid, h->block, 0, h->stream>>>((uint32_t*)words_dev, (double*)normals_dev, P);
+        debug_rng_kernel<double><<<h->grid, h->block, 0, h->stream>>>((uint32_t*)words_dev, (double*)normals_dev,
+                                                                     mismatch, t_hi, t_lo, P);
     } else {
         const StepParams<float> P = step_params<float>(h, step);
-        debug_rng_kernel<float><<<h->grid, h->block, 0, h->stream>>>((uint32_t*)words_dev, (float*)normals_dev, P);
+        debug_rng_kernel<float><<<h->grid, h->block, 0, h->stream>>>((uint32_t*)words_dev, (float*)normals_dev,
+                                                                    mismatch, t_hi, t_lo, P);
     }
-    return after_launch(h, "debug_rng_kernel");
+    rc = after_launch(h, "debug_rng_kernel");
+    if (rc != RFLBM_OK) return rc;
+    unsigned long long bad = 0;
+    rc = check_cuda(h, cudaMemcpyAsync(&bad, mismatch, sizeof(bad), cudaMemcpyDeviceToHost, h->stream), "cudaMemcpyAsync");
+    if (rc != RFLBM_OK) return rc;
+    rc = check_cuda(h, cudaStreamSynchronize(h->stream), "cudaStreamSynchronize");
+    if (rc != RFLBM_OK) return rc;
+    if (bad != 0) return fail(h, RFLBM_ECUDA, "hand-scheduled Philox differs from the ten-round loop at %llu sites", bad);
+    return RFLBM_OK;
 }
 
 // ---------------------------------------------------------------- host-buffer job (bench.py "e2e")

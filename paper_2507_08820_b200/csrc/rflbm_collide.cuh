@@ -10,9 +10,11 @@
 // What differs from a literal reading (same real function, different operation order):
 //   * D3Q27 is a tensor product, e_ki = H_p(cx) H_q(cy) H_r(cz), w_i = w1(cx) w1(cy) w1(cz), b_k = beta_p beta_q beta_r,
 //     so both transforms are done separably (three passes of 3-point 1-D transforms) instead of 27x27.
-//   * modes are carried ORTHONORMALISED, Mt_k = M_k / sqrt(b_k): the FDT amplitude (Eq.9) becomes the same
-//     sqrt(3 kT rho omega_k (2-omega_k)) for every mode, i.e. one scale for the 17 ghost modes, one for the 6
-//     stress modes, and the 1-D back-transform matrix is T[c][p] = w1(c) H_p(c) / sqrt(beta_p).
+//   * modes are carried SCALED, Ms[p][q][r] = M_k 2^-(number of non-zero exponents among p,q,r).  The 1-D
+//     back-transform f(c) = w1(c) sum_p H_p(c) m_p / beta_p is f(0) = 2/3 m0 - m2, f(+-1) = m0/6 +- m1/2 + m2/2;
+//     with m1, m2 pre-halved it costs 4 flops (e = m0/6 + m2s, f+- = e +- m1s, f0 = m0 - 2e) instead of 6, and
+//     the scaling is free: the equilibrium becomes rho prod (1, u/2, u^2/2), the stress and noise coefficients
+//     absorb it into constants.
 //   * only the 10 moments of order <= 2 are needed from the incoming populations (ghost modes are rebuilt from
 //     rho,u, not relaxed), so the forward transform is truncated.
 #pragma once
@@ -21,23 +23,45 @@
 
 namespace rflbm_dev {
 
+// noise amplitude classes: phi_k 2^-nnz / sqrt(rho) = sqrt(3 kT omega_k (2-omega_k)) prod_axis s_p with
+// s = sqrt(beta_p) 2^-[p>0] = (1, sqrt3/6, sqrt2/6); a class is the multiset of exponents of the mode
+enum { AMP_200 = 0, AMP_110, AMP_210, AMP_111, AMP_220, AMP_211, AMP_221, AMP_222, AMP_N };
+
+__host__ __device__ constexpr int amp_class(int p, int q, int r)
+{
+    const int n1 = (p == 1) + (q == 1) + (r == 1), n2 = (p == 2) + (q == 2) + (r == 2);
+    return (n2 == 1 && n1 == 0) ? AMP_200 : (n2 == 0 && n1 == 2) ? AMP_110 : (n2 == 1 && n1 == 1) ? AMP_210
+         : (n2 == 0 && n1 == 3) ? AMP_111 : (n2 == 2 && n1 == 0) ? AMP_220 : (n2 == 1 && n1 == 2) ? AMP_211
+         : (n2 == 2 && n1 == 1) ? AMP_221 : AMP_222;
+}
+
 template <typename real>
 struct StepParams {
     int nx, ny, nz;
     long long N;
-    real one_minus_omega;   // 1 - omega_h
-    real noise_ghost;       // sqrt(3 kT)                      (times sqrt(rho) at the site)
-    real noise_hydro;       // sqrt(3 kT omega_h (2-omega_h))
+    real half_omc;          // (1 - omega_h)/2
+    real amp[AMP_N];        // noise amplitude per class (times sqrt(rho) at the site), Eq.9
     real gx, gy, gz;        // acceleration (R13)
     real force_stress;      // 1 - omega_h/2
-    uint32_t t_hi, t_lo;    // step counter
-    PhiloxKeys keys;
-    const f64x2* tables;    // device: log table [256] then sin/cos table [256] (fp64 noise only)
+    PhiloxStep rng;         // round keys and the grid-uniform part of the first Philox rounds for this step
+    const f64x2* tables;    // device: log table [LOG_TABLE_N] then sin/cos table [SC_TABLE_N] (fp64 noise only)
 };
 
-template <typename real> __device__ __forceinline__ real rsqrt_real(real x);
-template <> __device__ __forceinline__ double rsqrt_real<double>(double x) { return rsqrt(x); }
-template <> __device__ __forceinline__ float rsqrt_real<float>(float x) { return rsqrtf(x); }
+// 1/x and sqrt(x) for x of order one (the density): approximate seed + Newton, no special cases
+template <typename real> __device__ __forceinline__ real rcp_pos(real x);
+template <> __device__ __forceinline__ double rcp_pos<double>(double x)
+{
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));       // 2^-20
+    double e = fma(-x, y, 1.0);
+    y = fma(y, e, y);                                            // 2^-40
+    e = fma(-x, y, 1.0);
+    return fma(y, e, y);                                         // < 1 ulp
+}
+template <> __device__ __forceinline__ float rcp_pos<float>(float x) { return 1.0f / x; }
+template <typename real> __device__ __forceinline__ real sqrt_rho(real x);
+template <> __device__ __forceinline__ double sqrt_rho<double>(double x) { return sqrt_pos(x); }
+template <> __device__ __forceinline__ float sqrt_rho<float>(float x) { return sqrtf(x); }
 
 // conserved moments + raw second moments of g[cz+1][cy+1][cx+1] (Eq.2-3, and sum g c_a c_b for Eq.19)
 template <typename real>
@@ -81,16 +105,14 @@ __device__ __forceinline__ Moments10<real> forward_moments(const real (&g)[3][3]
     return m;
 }
 
-// 1-D back-transform of orthonormal modes (m0,m1,m2) -> values at c = -1, 0, +1:
-//   T[c][p] = w1(c) H_p(c) / sqrt(beta_p):  c=0: (2/3, 0, -sqrt2/3);  c=+-1: (1/6, +-sqrt3/6, sqrt2/6)
+// 1-D back-transform of (m0, m1/2, m2/2) -> values at c = -1, 0, +1 (see the header comment)
 template <typename real>
-__device__ __forceinline__ void back1d(real m0, real m1, real m2, real& fm, real& f0, real& fp)
+__device__ __forceinline__ void back1d(real m0, real m1s, real m2s, real& fm, real& f0, real& fp)
 {
-    const real t = real(SQRT2 / 6.0) * m2;
-    const real e = fma(real(1.0 / 6.0), m0, t);
-    f0 = fma(real(-2.0), t, real(2.0 / 3.0) * m0);
-    fp = fma(real(SQRT3 / 6.0), m1, e);
-    fm = fma(real(-SQRT3 / 6.0), m1, e);
+    const real e = fma(real(1.0 / 6.0), m0, m2s);
+    fp = e + m1s;
+    fm = e - m1s;
+    f0 = fma(real(-2.0), e, m0);
 }
 
 // In: g = pre-collision populations of the site.  Out: g = post-collision populations f*.
@@ -101,40 +123,18 @@ __device__ __forceinline__ void collide(real (&g)[3][3][3], const StepParams<rea
     const Moments10<real> m = forward_moments(g);
 
     // Eq.3 (with the half-force shift of R13)
-    const real inv_rho = real(1.0) / m.rho;
+    const real inv_rho = rcp_pos<real>(m.rho);
     real ux = m.jx * inv_rho, uy = m.jy * inv_rho, uz = m.jz * inv_rho;
-    real Fx = real(0), Fy = real(0), Fz = real(0);
     if (FORCE) {
-        Fx = m.rho * P.gx; Fy = m.rho * P.gy; Fz = m.rho * P.gz;
         ux = fma(real(0.5), P.gx, ux); uy = fma(real(0.5), P.gy, uy); uz = fma(real(0.5), P.gz, uz);
     }
-    const real rux = m.rho * ux, ruy = m.rho * uy, ruz = m.rho * uz;
 
-    // Eq.19: a_1,ab = sum_i g_i (c_a c_b - delta_ab/3) - rho u_a u_b
-    const real third_rho = m.rho * real(1.0 / 3.0);
-    real axx = (m.pxx - third_rho) - rux * ux;
-    real ayy = (m.pyy - third_rho) - ruy * uy;
-    real azz = (m.pzz - third_rho) - ruz * uz;
-    real axy = m.pxy - rux * uy;
-    real axz = m.pxz - rux * uz;
-    real ayz = m.pyz - ruy * uz;
-    // relaxed: (1-omega_h) a_1 (+ Guo stress source (1-omega_h/2)(u_a F_b + u_b F_a))
-    axx *= P.one_minus_omega; ayy *= P.one_minus_omega; azz *= P.one_minus_omega;
-    axy *= P.one_minus_omega; axz *= P.one_minus_omega; ayz *= P.one_minus_omega;
-    if (FORCE) {
-        axx = fma(P.force_stress, real(2.0) * ux * Fx, axx);
-        ayy = fma(P.force_stress, real(2.0) * uy * Fy, ayy);
-        azz = fma(P.force_stress, real(2.0) * uz * Fz, azz);
-        axy = fma(P.force_stress, ux * Fy + uy * Fx, axy);
-        axz = fma(P.force_stress, ux * Fz + uz * Fx, axz);
-        ayz = fma(P.force_stress, uy * Fz + uz * Fy, ayz);
-    }
-
-    // Eq.20 in orthonormal form: Mt[p][q][r] = rho * (n_p ux^p)(n_q uy^q)(n_r uz^r)
-    real ex[3] = {real(1.0), real(NRM1) * ux, real(NRM2) * ux * ux};
-    real ey[3] = {real(1.0), real(NRM1) * uy, real(NRM2) * uy * uy};
-    real ez[3] = {real(1.0), real(NRM1) * uz, real(NRM2) * uz * uz};
-    real Mt[3][3][3];
+    // Eq.20, scaled: Ms[p][q][r] = rho X_p Y_q Z_r with X = (1, ux/2, ux^2/2)
+    const real hx = real(0.5) * ux, hy = real(0.5) * uy, hz = real(0.5) * uz;
+    const real ex[3] = {real(1.0), hx, hx * ux};
+    const real ey[3] = {real(1.0), hy, hy * uy};
+    const real ez[3] = {real(1.0), hz, hz * uz};
+    real Ms[3][3][3];
 #pragma unroll
     for (int p = 0; p < 3; ++p) {
         const real a = (p == 0) ? m.rho : m.rho * ex[p];
@@ -142,42 +142,62 @@ __device__ __forceinline__ void collide(real (&g)[3][3][3], const StepParams<rea
         for (int q = 0; q < 3; ++q) {
             const real ab = (q == 0) ? a : a * ey[q];
 #pragma unroll
-            for (int r = 0; r < 3; ++r) Mt[p][q][r] = (r == 0) ? ab : ab * ez[r];
+            for (int r = 0; r < 3; ++r) Ms[p][q][r] = (r == 0) ? ab : ab * ez[r];
         }
     }
-    // stress modes k = 4..9 (normalised by 1/sqrt(b_k): 3/sqrt2 for the diagonal, 3 for the off-diagonal ones)
-    Mt[2][0][0] = fma(real(NRM2), axx, Mt[2][0][0]);
-    Mt[0][2][0] = fma(real(NRM2), ayy, Mt[0][2][0]);
-    Mt[0][0][2] = fma(real(NRM2), azz, Mt[0][0][2]);
-    Mt[1][1][0] = fma(real(3.0), axy, Mt[1][1][0]);
-    Mt[1][0][1] = fma(real(3.0), axz, Mt[1][0][1]);
-    Mt[0][1][1] = fma(real(3.0), ayz, Mt[0][1][1]);
-    if (FORCE) {   // post-collision momentum j + F: modes 1..3 get another F/2 (times n_1)
-        Mt[1][0][0] = fma(real(0.5 * NRM1), Fx, Mt[1][0][0]);
-        Mt[0][1][0] = fma(real(0.5 * NRM1), Fy, Mt[0][1][0]);
-        Mt[0][0][1] = fma(real(0.5 * NRM1), Fz, Mt[0][0][1]);
+
+    // stress modes k = 4..9: Eq.19 a_1,ab = sum_i g_i (c_a c_b - delta_ab/3) - rho u_a u_b, relaxed by (1-omega_h)
+    // (Eq.26).  Scaled: diagonal E + (1-omega_h)/2 (p_aa - rho/3 - 2E), E = rho u_a^2/2;
+    //           off-diagonal E + (1-omega_h)/4 (p_ab - 4E), E = rho u_a u_b/4.
+    {
+        const real k2 = P.half_omc, k4 = real(0.5) * P.half_omc;
+        const real dxx = fma(real(-2.0), Ms[2][0][0], fma(real(-1.0 / 3.0), m.rho, m.pxx));
+        const real dyy = fma(real(-2.0), Ms[0][2][0], fma(real(-1.0 / 3.0), m.rho, m.pyy));
+        const real dzz = fma(real(-2.0), Ms[0][0][2], fma(real(-1.0 / 3.0), m.rho, m.pzz));
+        Ms[2][0][0] = fma(k2, dxx, Ms[2][0][0]);
+        Ms[0][2][0] = fma(k2, dyy, Ms[0][2][0]);
+        Ms[0][0][2] = fma(k2, dzz, Ms[0][0][2]);
+        Ms[1][1][0] = fma(k4, fma(real(-4.0), Ms[1][1][0], m.pxy), Ms[1][1][0]);
+        Ms[1][0][1] = fma(k4, fma(real(-4.0), Ms[1][0][1], m.pxz), Ms[1][0][1]);
+        Ms[0][1][1] = fma(k4, fma(real(-4.0), Ms[0][1][1], m.pyz), Ms[0][1][1]);
+    }
+    if (FORCE) {
+        // Guo forcing in moment form (R13): post-collision momentum j + F (modes 1..3 get another F/2, scaled 1/2),
+        // stress source (1-omega_h/2)(u_a F_b + u_b F_a) (scaled 1/2 diagonal, 1/4 off-diagonal)
+        const real Fx = m.rho * P.gx, Fy = m.rho * P.gy, Fz = m.rho * P.gz;
+        Ms[1][0][0] = fma(real(0.25), Fx, Ms[1][0][0]);
+        Ms[0][1][0] = fma(real(0.25), Fy, Ms[0][1][0]);
+        Ms[0][0][1] = fma(real(0.25), Fz, Ms[0][0][1]);
+        const real fs = P.force_stress, fq = real(0.25) * P.force_stress;
+        Ms[2][0][0] = fma(fs, ux * Fx, Ms[2][0][0]);
+        Ms[0][2][0] = fma(fs, uy * Fy, Ms[0][2][0]);
+        Ms[0][0][2] = fma(fs, uz * Fz, Ms[0][0][2]);
+        Ms[1][1][0] = fma(fq, fma(ux, Fy, uy * Fx), Ms[1][1][0]);
+        Ms[1][0][1] = fma(fq, fma(ux, Fz, uz * Fx), Ms[1][0][1]);
+        Ms[0][1][1] = fma(fq, fma(uy, Fz, uz * Fy), Ms[0][1][1]);
     }
 
-    // Eq.8-9: noise on k = 4..26, Mt_k += sqrt(3 kT rho omega_k(2-omega_k)) r_k
+    // Eq.8-9: noise on k = 4..26, Ms_k += sqrt(rho) amp[class(k)] r_k
     if (NOISE) {
-        const real sq_rho = m.rho * rsqrt_real<real>(m.rho);
-        const real amp_h = sq_rho * P.noise_hydro;
-        const real amp_g = sq_rho * P.noise_ghost;
+        const real sq_rho = sqrt_rho<real>(m.rho);
+        real amp[AMP_N];
+#pragma unroll
+        for (int n = 0; n < AMP_N; ++n) amp[n] = sq_rho * P.amp[n];
+        const PhiloxSite ps = philox_site(site, P.rng);
 #pragma unroll
         for (int call = 0; call < 6; ++call) {
             uint32_t w[4];
-            philox4x32_10(site, P.t_hi, P.t_lo, (uint32_t)call, P.keys, w);
+            philox_call(ps, P.rng, call, w);
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
                 real z0, z1;
                 normal_pair(w[2 * h], w[2 * h + 1], lg, sc, z0, z1);
                 const int k = 4 + 4 * call + 2 * h;            // modes k (first) and k+1 (second), R8
-                const real amp = (k <= 9) ? amp_h : amp_g;      // pairs (4,5),(6,7),(8,9) are all-stress
-                real& m0 = Mt[mode_p(k)][mode_q(k)][mode_r(k)];
-                m0 = fma(amp, z0, m0);
+                real& m0 = Ms[mode_p(k)][mode_q(k)][mode_r(k)];
+                m0 = fma(amp[amp_class(mode_p(k), mode_q(k), mode_r(k))], z0, m0);
                 if (k + 1 < Q) {
-                    real& m1 = Mt[mode_p(k + 1)][mode_q(k + 1)][mode_r(k + 1)];
-                    m1 = fma(amp, z1, m1);
+                    real& m1 = Ms[mode_p(k + 1)][mode_q(k + 1)][mode_r(k + 1)];
+                    m1 = fma(amp[amp_class(mode_p(k + 1), mode_q(k + 1), mode_r(k + 1))], z1, m1);
                 }
             }
         }
@@ -188,7 +208,7 @@ __device__ __forceinline__ void collide(real (&g)[3][3][3], const StepParams<rea
 #pragma unroll
     for (int p = 0; p < 3; ++p)
 #pragma unroll
-        for (int q = 0; q < 3; ++q) back1d(Mt[p][q][0], Mt[p][q][1], Mt[p][q][2], A[p][q][0], A[p][q][1], A[p][q][2]);
+        for (int q = 0; q < 3; ++q) back1d(Ms[p][q][0], Ms[p][q][1], Ms[p][q][2], A[p][q][0], A[p][q][1], A[p][q][2]);
     real B[3][3][3];   // [p][cy][cz]
 #pragma unroll
     for (int p = 0; p < 3; ++p)

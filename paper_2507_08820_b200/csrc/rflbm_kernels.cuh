@@ -249,20 +249,27 @@ init_kernel(const real* __restrict__ rho, const real* __restrict__ u, double rho
     }
 }
 
-// test hook: the words and normals the step kernel draws at (t_hi,t_lo)
+// test hook: the words and normals the step kernel draws at step (t_hi,t_lo).  The words come from the
+// hand-scheduled philox_call() of the step kernel; mismatch[0] counts sites where they differ from the textbook
+// ten-round loop philox4x32_10() (must stay 0).
 template <typename real>
 __global__ void __launch_bounds__(128)
-debug_rng_kernel(uint32_t* __restrict__ words, real* __restrict__ normals, const __grid_constant__ StepParams<real> P)
+debug_rng_kernel(uint32_t* __restrict__ words, real* __restrict__ normals, unsigned long long* __restrict__ mismatch,
+                 uint32_t t_hi, uint32_t t_lo, const __grid_constant__ StepParams<real> P)
 {
     constexpr bool TABLES = sizeof(real) == 8;
     __shared__ f64x2 s_tab[TABLES ? LOG_TABLE_N + SC_TABLE_N : 1];
     if (TABLES) stage_tables(P.tables, s_tab);
     const SiteIndex i = my_site(P.nx, P.ny);
     if (!i.valid) return;
+    const PhiloxSite ps = philox_site((uint32_t)i.s, P.rng);
+    bool bad = false;
 #pragma unroll
     for (int call = 0; call < 6; ++call) {
-        uint32_t w[4];
-        philox4x32_10((uint32_t)i.s, P.t_hi, P.t_lo, (uint32_t)call, P.keys, w);
+        uint32_t w[4], w_ref[4];
+        philox_call(ps, P.rng, call, w);
+        philox4x32_10((uint32_t)i.s, t_hi, t_lo, (uint32_t)call, P.rng, w_ref);
+        bad = bad || w[0] != w_ref[0] || w[1] != w_ref[1] || w[2] != w_ref[2] || w[3] != w_ref[3];
         if (words != nullptr)
 #pragma unroll
             for (int mth = 0; mth < 4; ++mth) words[(long long)(4 * call + mth) * P.N + i.s] = w[mth];
@@ -276,6 +283,7 @@ debug_rng_kernel(uint32_t* __restrict__ words, real* __restrict__ normals, const
                 if (k + 1 < Q) normals[(long long)(k + 1 - 4) * P.N + i.s] = z1;
             }
     }
+    if (bad) atomicAdd(mismatch, 1ull);
 }
 
 }  // namespace rflbm_dev

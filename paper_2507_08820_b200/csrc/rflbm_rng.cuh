@@ -3,6 +3,15 @@
 // "r_k is a standard normal random variable"; generator and mapping are this build's reading:
 // Philox4x32-10 (Salmon et al., SC'11), key = (seed lo, seed hi), counter = (site, t>>32, t&0xffffffff, call),
 // 6 calls per site and step -> 24 words -> 12 Box-Muller pairs -> the 23 normals of modes k = 4..26.
+//
+// The six calls of a site differ only in counter word 3, and two of the four counter words (t_hi, t_lo) and the
+// key are the same for the whole grid.  Following the data flow of the first three rounds by hand:
+//   round 1: M1*t_lo is grid-uniform, M0*site is shared by the six calls  -> one XOR per call
+//   round 2: M0*(uniform) is grid-uniform                                  -> one IMAD.WIDE + one XOR per call (+1 shared XOR)
+//   round 3: M1*(shared)  is shared by the six calls                       -> one IMAD.WIDE + two XOR per call (+1 shared IMAD)
+// so the host precomputes the uniform pieces once per step (PhiloxStep) and a site spends 34 instead of 40
+// integer instructions per call.  The words are bit-identical to the textbook loop (philox4x32_10 below, which
+// the debug kernel cross-checks against in tests/test_gpu_parity.py).
 #pragma once
 #include <cstdint>
 
@@ -10,34 +19,98 @@
 
 namespace rflbm_dev {
 
-struct PhiloxKeys {
-    uint32_t k0[10];  // round keys key0 + r*0x9E3779B9 (precomputed on the host: uniform over the grid)
-    uint32_t k1[10];  // key1 + r*0xBB67AE85
+constexpr uint32_t PHILOX_M0 = 0xD2511F53u, PHILOX_M1 = 0xCD9E8D57u;
+constexpr uint32_t PHILOX_W0 = 0x9E3779B9u, PHILOX_W1 = 0xBB67AE85u;
+
+struct PhiloxStep {
+    uint32_t k0[10];   // round keys key0 + r*W0
+    uint32_t k1[10];   // key1 + r*W1
+    uint32_t r1x[6];   // call ^ k1[0]                                  (round 1: n2 = hi(M0*site) ^ r1x[call])
+    uint32_t r2_c0;    // round-2 c0 = hi(M1*t_lo) ^ t_hi ^ k0[0]       (only its products are used below)
+    uint32_t r2_n0x;   // lo(M1*t_lo) ^ k0[1]                           (round 2: n0 = hi(M1*c2) ^ r2_n0x)
+    uint32_t r2_n2x;   // hi(M0*r2_c0) ^ k1[1]                          (round 2: n2 = lo(M0*site) ^ r2_n2x)
+    uint32_t r3_n2x;   // lo(M0*r2_c0) ^ k1[2]                          (round 3: n2 = hi(M0*c0) ^ r3_n2x)
 };
 
-__host__ inline PhiloxKeys make_philox_keys(uint64_t seed)
+__host__ inline PhiloxStep make_philox_step(uint64_t seed, uint64_t t)
 {
-    PhiloxKeys k;
+    PhiloxStep s;
     uint32_t a = (uint32_t)(seed & 0xFFFFFFFFu), b = (uint32_t)(seed >> 32);
     for (int r = 0; r < 10; ++r) {
-        k.k0[r] = a;
-        k.k1[r] = b;
-        a += 0x9E3779B9u;
-        b += 0xBB67AE85u;
+        s.k0[r] = a;
+        s.k1[r] = b;
+        a += PHILOX_W0;
+        b += PHILOX_W1;
     }
-    return k;
+    const uint32_t t_hi = (uint32_t)(t >> 32), t_lo = (uint32_t)(t & 0xFFFFFFFFu);
+    const uint64_t p1 = (uint64_t)PHILOX_M1 * t_lo;
+    for (uint32_t q = 0; q < 6; ++q) s.r1x[q] = q ^ s.k1[0];
+    s.r2_c0 = (uint32_t)(p1 >> 32) ^ t_hi ^ s.k0[0];
+    s.r2_n0x = (uint32_t)p1 ^ s.k0[1];
+    const uint64_t p0 = (uint64_t)PHILOX_M0 * s.r2_c0;
+    s.r2_n2x = (uint32_t)(p0 >> 32) ^ s.k1[1];
+    s.r3_n2x = (uint32_t)p0 ^ s.k1[2];
+    return s;
 }
 
-// one Philox4x32-10 block; 2 IMAD.WIDE.U32 + 2 LOP3 per round
-__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, const PhiloxKeys& key,
+// textbook Philox4x32-10 block (test hook only): 2 IMAD.WIDE.U32 + 2 LOP3 per round
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, const PhiloxStep& key,
                                               uint32_t (&out)[4])
 {
 #pragma unroll
     for (int r = 0; r < 10; ++r) {
-        const uint64_t p0 = (uint64_t)0xD2511F53u * (uint64_t)c0;
-        const uint64_t p1 = (uint64_t)0xCD9E8D57u * (uint64_t)c2;
+        const uint64_t p0 = (uint64_t)PHILOX_M0 * (uint64_t)c0;
+        const uint64_t p1 = (uint64_t)PHILOX_M1 * (uint64_t)c2;
         const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ key.k0[r];
         const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ key.k1[r];
+        c1 = (uint32_t)p1;
+        c3 = (uint32_t)p0;
+        c0 = n0;
+        c2 = n2;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// The part of the six calls that does not depend on the call index (see the header comment).
+struct PhiloxSite {
+    uint32_t p0_hi;    // hi(M0*site)
+    uint32_t r3_c2;    // round-3 c2 = lo(M0*site) ^ r2_n2x
+    uint32_t r3_p1_hi, r3_p1_lo;   // M1 * r3_c2
+};
+
+__device__ __forceinline__ PhiloxSite philox_site(uint32_t site, const PhiloxStep& S)
+{
+    PhiloxSite P;
+    const uint64_t p0 = (uint64_t)PHILOX_M0 * (uint64_t)site;
+    P.p0_hi = (uint32_t)(p0 >> 32);
+    P.r3_c2 = (uint32_t)p0 ^ S.r2_n2x;
+    const uint64_t p1 = (uint64_t)PHILOX_M1 * (uint64_t)P.r3_c2;
+    P.r3_p1_hi = (uint32_t)(p1 >> 32);
+    P.r3_p1_lo = (uint32_t)p1;
+    return P;
+}
+
+// call `call` (0..5) of the site: identical words to philox4x32_10(site, t_hi, t_lo, call)
+__device__ __forceinline__ void philox_call(const PhiloxSite& P, const PhiloxStep& S, int call, uint32_t (&out)[4])
+{
+    // round 1 -> (c0, c1, c2, c3) = (uniform, uniform, n2, lo(M0*site))
+    const uint32_t r2_c2 = P.p0_hi ^ S.r1x[call];
+    // round 2
+    const uint64_t q1 = (uint64_t)PHILOX_M1 * (uint64_t)r2_c2;
+    uint32_t c0 = (uint32_t)(q1 >> 32) ^ S.r2_n0x;
+    uint32_t c1 = (uint32_t)q1;
+    // round 3: c2 = P.r3_c2 (shared), c3 = lo(M0*r2_c0) (uniform, folded into r3_n2x)
+    const uint64_t q0 = (uint64_t)PHILOX_M0 * (uint64_t)c0;
+    c0 = P.r3_p1_hi ^ c1 ^ S.k0[2];
+    uint32_t c2 = (uint32_t)(q0 >> 32) ^ S.r3_n2x;
+    c1 = P.r3_p1_lo;
+    uint32_t c3 = (uint32_t)q0;
+#pragma unroll
+    for (int r = 3; r < 10; ++r) {
+        const uint64_t p0 = (uint64_t)PHILOX_M0 * (uint64_t)c0;
+        const uint64_t p1 = (uint64_t)PHILOX_M1 * (uint64_t)c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ S.k0[r];
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ S.k1[r];
         c1 = (uint32_t)p1;
         c3 = (uint32_t)p0;
         c0 = n0;

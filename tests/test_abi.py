@@ -40,7 +40,7 @@ def test_create_validation_and_workspace_size(lib):
     assert lib.rflbm_create(4, 4, 4, 1.0, 0.0, 1.0, 0, 5, C.byref(h)) == binding.EINVAL
     assert lib.rflbm_create(4, 4, 4, 1.0, 0.0, 1.0, 0, binding.F64, None) == binding.EINVAL
     assert lib.rflbm_create(16, 16, 16, 1.0, 1e-4, 1.0, 42, binding.F64, C.byref(h)) == binding.OK
-    assert lib.rflbm_workspace_bytes(h) == 2 * 27 * 4096 * 8 + 4096 + 8192
+    assert lib.rflbm_workspace_bytes(h) == 2 * 27 * 4096 * 8 + 4096 + 12288
     # state machine, host side only
     assert lib.rflbm_step(h, 1) == binding.ESTATE
     assert b"before init" in lib.rflbm_last_error(h)
@@ -52,7 +52,7 @@ def test_create_validation_and_workspace_size(lib):
     assert lib.rflbm_destroy(h) == binding.OK
     h32 = C.c_void_p()
     assert lib.rflbm_create(4, 4, 2, 1.0, 0.0, 1.0, 0, binding.F32, C.byref(h32)) == binding.OK
-    assert lib.rflbm_workspace_bytes(h32) == 2 * 3584 + 4096 + 8192                  # 27*32*4 = 3456 -> 256-aligned 3584
+    assert lib.rflbm_workspace_bytes(h32) == 2 * 3584 + 4096 + 12288                  # 27*32*4 = 3456 -> 256-aligned 3584
     assert lib.rflbm_set_walls_z(h32, 1) == binding.EINVAL                     # nz < 3
     lib.rflbm_destroy(h32)
 
