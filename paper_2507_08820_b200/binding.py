@@ -15,7 +15,7 @@ KERNEL_AUTO, KERNEL_PLAIN, KERNEL_TMA = 0, 1, 2
 Q = 27
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "csrc", "librflbm.so")
+LIB_PATH = os.environ.get("RFLBM_LIB") or os.path.join(_HERE, "csrc", "librflbm.so")   # env: development builds
 _lib = None
 
 # every symbol include/rflbm.h declares: name -> (restype, argtypes)

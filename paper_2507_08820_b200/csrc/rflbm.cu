@@ -7,6 +7,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -19,6 +20,7 @@ using namespace rflbm_dev;
 struct rflbm {
     int nx, ny, nz;
     long long N;
+    long long QS;        // elements between population arrays inside a buffer: N rounded up to 32 plus padding
     double tau, kT, rho0;
     uint64_t seed;
     int precision;
@@ -39,12 +41,12 @@ struct rflbm {
     CUtensorMap tmap[2];  // TMA descriptors of the two population buffers (fp64, nx >= 128, nx even)
     bool tma_ok;
     int variant;          // RFLBM_KERNEL_AUTO / _PLAIN / _TMA
-    int rows_per_block;   // y rows walked by one block of the TMA kernel
+    int tma_rows;         // y rows walked by one block of the TMA kernel
     char err[512];
 };
 
 static size_t real_size(const rflbm* h) { return h->precision == RFLBM_F64 ? sizeof(double) : sizeof(float); }
-static size_t pop_bytes(const rflbm* h) { return (size_t)Q * (size_t)h->N * real_size(h); }
+static size_t pop_bytes(const rflbm* h) { return (size_t)Q * (size_t)h->QS * real_size(h); }
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 static constexpr size_t TABLE_BYTES = (LOG_TABLE_N + SC_TABLE_N) * sizeof(f64x2);
 
@@ -77,7 +79,7 @@ typedef CUresult (*encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_
                                     const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                     CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-// 4-D view [27][nz][ny][nx] of one fp64 population buffer, box = BOX_X consecutive x of one row of one array
+// 4-D view [27][nz][ny][nx] of one fp64 population buffer, box = BOX_X consecutive x of one row of BOX_Q arrays
 static bool make_tensor_map(rflbm* h, void* base, CUtensorMap* out)
 {
     void* fn = nullptr;
@@ -88,8 +90,8 @@ static bool make_tensor_map(rflbm* h, void* base, CUtensorMap* out)
         return false;
     }
     const cuuint64_t dims[4] = {(cuuint64_t)h->nx, (cuuint64_t)h->ny, (cuuint64_t)h->nz, (cuuint64_t)Q};
-    const cuuint64_t strides[3] = {(cuuint64_t)h->nx * 8, (cuuint64_t)h->nx * h->ny * 8, (cuuint64_t)h->N * 8};
-    const cuuint32_t box[4] = {BOX_X, 1, 1, 1};   // 130 elements: 16-byte aligned starts, see rflbm_step_tma.cuh
+    const cuuint64_t strides[3] = {(cuuint64_t)h->nx * 8, (cuuint64_t)h->nx * h->ny * 8, (cuuint64_t)h->QS * 8};
+    const cuuint32_t box[4] = {BOX_X, 1, 1, BOX_Q};   // 132 x 3 elements: 16-byte aligned starts, see rflbm_step_tma.cuh
     const cuuint32_t estr[4] = {1, 1, 1, 1};
     const CUresult r = ((encode_tiled_fn)fn)(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box, estr,
                                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
@@ -114,6 +116,13 @@ extern "C" int rflbm_create(int nx, int ny, int nz, double tau, double kT, doubl
     memset(h, 0, sizeof(*h));
     h->nx = nx; h->ny = ny; h->nz = nz;
     h->N = (long long)nx * ny * nz;
+    // Population arrays are NOT packed back to back: for power-of-two lattices N*sizeof(real) is a power of two
+    // and the 27 read streams + 27 write streams of a step would all hit the same DRAM channel/bank residues.
+    // A pad of 37 x 256 B skews successive arrays; small lattices only round up to 32.
+    long long pad = (h->N >= (1 << 16)) ? 37 * 32 : 0;
+    if (const char* e = getenv("RFLBM_QPAD")) pad = atoll(e) / 32 * 32;          // development knob (bench sweeps)
+    h->QS = (h->N + 31) / 32 * 32 + pad;
+    if ((double)h->QS >= 4294967296.0) { delete h; return RFLBM_EINVAL; }
     h->tau = tau; h->kT = kT; h->rho0 = rho0; h->seed = seed; h->precision = precision;
     // one thread per site; a warp covers 32 consecutive x whenever nx >= 32
     int bx = 8;
@@ -121,7 +130,11 @@ extern "C" int rflbm_create(int nx, int ny, int nz, double tau, double kT, doubl
     const int by = 128 / bx;
     h->block = dim3(bx, by, 1);
     h->grid = dim3((nx + bx - 1) / bx, (ny + by - 1) / by, nz);
-    h->rows_per_block = 16;
+    h->tma_rows = 16;
+    if (const char* e = getenv("RFLBM_TMA_ROWS")) {           // development knob (bench sweeps)
+        const int r = atoi(e);
+        if (r >= 1 && r <= 65536) h->tma_rows = r;
+    }
     *out = h;
     return RFLBM_OK;
 }
@@ -148,14 +161,16 @@ extern "C" int rflbm_set_workspace(rflbm_t* h, void* dev_ptr, size_t bytes)
     h->tables = (f64x2*)((char*)dev_ptr + 2 * pb + 4096);
     h->cur = 0;
     h->inited = false;
-    // the only device write outside the stream: upload the Box-Muller tables (host-generated, long double libm)
+    if (int rc0 = check_cuda(h, cudaMemset(h->acc, 0, 4096), "scratch clear")) return rc0;
+    // the only device writes outside the stream: the scratch clear above and the Box-Muller tables
+    // (host-generated, long double libm)
     static f64x2 host_tab[LOG_TABLE_N + SC_TABLE_N];
     fill_normal_tables(host_tab, host_tab + LOG_TABLE_N);
     const int rc = check_cuda(h, cudaMemcpy(h->tables, host_tab, TABLE_BYTES, cudaMemcpyHostToDevice), "table upload");
     if (rc != RFLBM_OK) return rc;
     // TMA path: fp64, rows of at least one 128-site tile, row pitch a multiple of 16 bytes
     h->tma_ok = false;
-    if (h->precision == RFLBM_F64 && h->nx >= TILE_X && h->nx % 2 == 0)
+    if (h->precision == RFLBM_F64 && h->nx >= TMA_MIN_NX && h->nx % 2 == 0)
         h->tma_ok = make_tensor_map(h, h->buf[0], &h->tmap[0]) && make_tensor_map(h, h->buf[1], &h->tmap[1]);
     return RFLBM_OK;
 }
@@ -189,7 +204,7 @@ template <typename real>
 static FieldParams<real> field_params(const rflbm* h)
 {
     FieldParams<real> P;
-    P.nx = h->nx; P.ny = h->ny; P.nz = h->nz; P.N = h->N;
+    P.nx = h->nx; P.ny = h->ny; P.nz = h->nz; P.N = h->N; P.QS = h->QS;
     P.hgx = (real)(0.5 * h->g[0]); P.hgy = (real)(0.5 * h->g[1]); P.hgz = (real)(0.5 * h->g[2]);
     P.walls = h->walls;
     return P;
@@ -200,7 +215,7 @@ static StepParams<real> step_params(const rflbm* h, uint64_t t)
 {
     StepParams<real> P;
     const double omega = 1.0 / h->tau;
-    P.nx = h->nx; P.ny = h->ny; P.nz = h->nz; P.N = h->N;
+    P.nx = h->nx; P.ny = h->ny; P.nz = h->nz; P.N = h->N; P.QS = h->QS;
     P.half_omc = (real)(0.5 * (1.0 - omega));
     // Eq.9 per unit sqrt(rho): sqrt(3 kT omega_k (2 - omega_k)) prod_axis s_p, s = (1, sqrt3/6, sqrt2/6)
     const double nh = std::sqrt(3.0 * h->kT * omega * (2.0 - omega)), ng = std::sqrt(3.0 * h->kT);
@@ -301,9 +316,9 @@ static void launch_step(rflbm* h, const StepParams<real>& P)
 template <bool WALLS, bool FORCE, bool NOISE>
 static void launch_step_tma(rflbm* h, const StepParams<double>& P)
 {
-    const dim3 grid((h->nx + TILE_X - 1) / TILE_X, (h->ny + h->rows_per_block - 1) / h->rows_per_block, h->nz);
+    const dim3 grid((h->nx + TILE_X - 1) / TILE_X, (h->ny + h->tma_rows - 1) / h->tma_rows, h->nz);
     step_kernel_tma<WALLS, FORCE, NOISE><<<grid, TILE_X, 0, h->stream>>>(
-        h->tmap[h->cur], (const double*)h->buf[h->cur], (double*)h->buf[h->cur ^ 1], P, h->rows_per_block);
+        h->tmap[h->cur], (const double*)h->buf[h->cur], (double*)h->buf[h->cur ^ 1], P, h->tma_rows);
 }
 
 static bool use_tma(const rflbm* h) { return h->tma_ok && h->variant != RFLBM_KERNEL_PLAIN; }

@@ -39,6 +39,7 @@ template <typename real>
 struct StepParams {
     int nx, ny, nz;
     long long N;
+    long long QS;           // elements between consecutive population arrays (N + padding, see rflbm.cu)
     real half_omc;          // (1 - omega_h)/2
     real amp[AMP_N];        // noise amplitude per class (times sqrt(rho) at the site), Eq.9
     real gx, gy, gz;        // acceleration (R13)

@@ -30,7 +30,7 @@ __device__ __forceinline__ SiteIndex my_site(int nx, int ny)
 
 // Pull-gather of the 27 pre-collision populations of a site into g[cz+1][cy+1][cx+1].
 template <typename real, bool WALLS>
-__device__ __forceinline__ void gather(const real* __restrict__ src, long long N, int nx, int ny, int nz,
+__device__ __forceinline__ void gather(const real* __restrict__ src, long long QS, int nx, int ny, int nz,
                                        const SiteIndex& i, real (&g)[3][3][3])
 {
     // neighbour coordinates x - cx etc. with periodic wrap; index a = cx+1 reads from xs[a]
@@ -48,8 +48,8 @@ __device__ __forceinline__ void gather(const real* __restrict__ src, long long N
 #pragma unroll
             for (int a = 0; a < 3; ++a) {
                 const int q = a + 3 * b + 9 * c;
-                const long long pull = (long long)q * N + row + xs[a];
-                const long long back = (long long)(26 - q) * N + i.s;
+                const long long pull = (long long)q * QS + row + xs[a];
+                const long long back = (long long)(26 - q) * QS + i.s;
                 g[c][b][a] = __ldg(src + ((WALLS && bounce) ? back : pull));
             }
         }
@@ -79,14 +79,14 @@ step_kernel(const real* __restrict__ src, real* __restrict__ dst, const __grid_c
     if (!i.valid) return;
     if (WALLS && (i.z == 0 || i.z == P.nz - 1)) return;    // solid layers are never updated
     real g[3][3][3];
-    gather<real, WALLS>(src, P.N, P.nx, P.ny, P.nz, i, g);
+    gather<real, WALLS>(src, P.QS, P.nx, P.ny, P.nz, i, g);
     collide<real, FORCE, NOISE>(g, P, (uint32_t)i.s, s_tab, s_tab + LOG_TABLE_N);
 #pragma unroll
     for (int c = 0; c < 3; ++c)
 #pragma unroll
         for (int b = 0; b < 3; ++b)
 #pragma unroll
-            for (int a = 0; a < 3; ++a) __stcs(dst + (long long)(a + 3 * b + 9 * c) * P.N + i.s, g[c][b][a]);
+            for (int a = 0; a < 3; ++a) __stcs(dst + (long long)(a + 3 * b + 9 * c) * P.QS + i.s, g[c][b][a]);
 }
 
 // ---------------------------------------------------------------- observables
@@ -94,6 +94,7 @@ template <typename real>
 struct FieldParams {
     int nx, ny, nz;
     long long N;
+    long long QS;         // elements between consecutive population arrays of the internal storage (>= N)
     real hgx, hgy, hgz;   // g/2: reported velocity u = j/rho + g/2 (R13)
     int walls;
 };
@@ -109,7 +110,7 @@ moments_kernel(const real* __restrict__ src, real* __restrict__ rho, real* __res
         return;
     }
     real g[3][3][3];
-    gather<real, WALLS>(src, P.N, P.nx, P.ny, P.nz, i, g);
+    gather<real, WALLS>(src, P.QS, P.nx, P.ny, P.nz, i, g);
     const Moments10<real> m = forward_moments(g);
     const real inv = real(1.0) / m.rho;
     rho[i.s] = m.rho;
@@ -130,7 +131,7 @@ diagnostics_kernel(const real* __restrict__ src, double* __restrict__ acc, const
     const bool fluid = i.valid && !(WALLS && (i.z == 0 || i.z == P.nz - 1));
     if (fluid) {
         real g[3][3][3];
-        gather<real, WALLS>(src, P.N, P.nx, P.ny, P.nz, i, g);
+        gather<real, WALLS>(src, P.QS, P.nx, P.ny, P.nz, i, g);
         const Moments10<real> m = forward_moments(g);
         const double rho = (double)m.rho;
         const double ux = (double)m.jx / rho + (double)P.hgx;
@@ -168,11 +169,11 @@ export_kernel(const real* __restrict__ src, real* __restrict__ out, const FieldP
     if (!i.valid) return;
     if (WALLS && (i.z == 0 || i.z == P.nz - 1)) {
 #pragma unroll
-        for (int n = 0; n < Q; ++n) out[(long long)n * P.N + i.s] = src[(long long)lex_of_canon(n) * P.N + i.s];
+        for (int n = 0; n < Q; ++n) out[(long long)n * P.N + i.s] = src[(long long)lex_of_canon(n) * P.QS + i.s];
         return;
     }
     real g[3][3][3];
-    gather<real, WALLS>(src, P.N, P.nx, P.ny, P.nz, i, g);
+    gather<real, WALLS>(src, P.QS, P.nx, P.ny, P.nz, i, g);
 #pragma unroll
     for (int n = 0; n < Q; ++n)
         out[(long long)n * P.N + i.s] = g[canon_cz(n) + 1][canon_cy(n) + 1][canon_cx(n) + 1];
@@ -204,8 +205,8 @@ import_kernel(const real* __restrict__ in, real* __restrict__ bufA, real* __rest
             }
         }
         const real v = in[from];
-        bufA[(long long)q * P.N + i.s] = v;
-        bufB[(long long)q * P.N + i.s] = v;
+        bufA[(long long)q * P.QS + i.s] = v;
+        bufB[(long long)q * P.QS + i.s] = v;
     }
 }
 
@@ -244,8 +245,8 @@ init_kernel(const real* __restrict__ rho, const real* __restrict__ u, double rho
             r = (double)rho[s]; ux = (double)u[s]; uy = (double)u[P.N + s]; uz = (double)u[2 * P.N + s];
         }
         const real v = (real)(r * phi1d(cx, ux) * phi1d(cy, uy) * phi1d(cz, uz));
-        bufA[(long long)q * P.N + i.s] = v;
-        bufB[(long long)q * P.N + i.s] = v;
+        bufA[(long long)q * P.QS + i.s] = v;
+        bufB[(long long)q * P.QS + i.s] = v;
     }
 }
 

@@ -2,21 +2,26 @@
 // nx >= 128, nx even.
 //
 // Why (profiles/r01a_*): in the plain one-thread-per-site kernel every one of the 27 neighbour loads costs 4-5
-// integer instructions of per-thread 64-bit address arithmetic and the block's memory latency is exposed
-// between its load phase and its ~1500-instruction compute phase.  Here the 27 row segments a tile of 128
-// consecutive x needs are fetched by 27 `cp.async.bulk.tensor` (TMA) copies issued by one thread into shared
-// memory: the TMA unit generates the addresses, applies the -c_q shift (box start x0 + c-shift, y -+ 1, z -+ 1,
-// array q — or array 26-q at the same site for halfway bounce-back, R12), and the copy of tile k+1 is issued as
-// soon as tile k has been moved from shared memory to registers, so it overlaps the whole collision of tile k.
-// Threads read their 27 populations with LDS [reg + immediate].  A block walks `rows` consecutive y rows so the
-// Box-Muller tables are staged once per block.
+// integer instructions of per-thread 64-bit address arithmetic, and a block's memory latency is exposed between
+// its load phase and its ~1300-instruction compute phase.  Here a tile is 128 consecutive x of one row; the 27
+// row segments it needs arrive as NINE `cp.async.bulk.tensor` copies (box = 132 x, 1 y, 1 z, 3 populations: the
+// three q = 3b+9c+{0,1,2} that share the source row (y-cy, z-cz)), issued by one elected thread of warp 0 into
+// shared memory.  The TMA unit generates the addresses, applies the y/z shift and the periodic wrap in y and z
+// (and fetches the opposite populations 26-q at the site itself for halfway bounce-back, R12); the copy of row
+// y+1 is issued as soon as row y has been moved from shared memory to registers, so it overlaps the whole
+// collision of row y.  Threads read their 27 populations with LDS [tid*8 + immediate].  A block walks `rows`
+// consecutive y rows, so the Box-Muller tables are staged once per block.
 //
-// TMA needs 16-byte aligned box starts (measured: an odd fp64 x coordinate raises "illegal instruction"), so every
-// copy is a 130-element box starting at an even x: [x0, x0+130) for cx <= 0 and [x0-2, x0+128) for cx = +1, and a
-// thread reads element tid + 1 of it for cx != 0 (tid for cx = 0 and for bounced-back populations).
+// TMA needs 16-byte aligned box starts, so a box starts at the even x0-2 and spans 132 elements; the thread at
+// x reads element tid+3 (cx=-1, source x+1), tid+2 (cx=0) or tid+1 (cx=+1, source x-1) of its row.
+// The one thing TMA cannot do is the periodic wrap in x (out-of-bounds box elements are zero-filled): the two
+// threads at x = 0 and x = nx-1 load their 9 wrapped populations directly from global memory, issued before the
+// mbarrier wait so that the latency hides behind it.
 //
-// The only thing TMA cannot do is the periodic wrap in x (out-of-bounds box elements are zero-filled): the
-// threads at x = 0 and x = nx-1 re-load their 9 wrapped populations directly from global memory.
+// Variants that were measured and dropped (512^3, kT=1e-4): one private 32-site pipeline per
+// warp (no block barrier, but 4x the TMA issue work and 12 % more L2->SM traffic: no faster); a persistent grid
+// with static or ticket-based strip assignment (1.1-1.5x SLOWER: warps of a block drift apart, the 16-byte halos
+// of neighbouring tiles stop hitting in L2).
 #pragma once
 #include <cuda.h>
 
@@ -24,9 +29,13 @@
 
 namespace rflbm_dev {
 
-constexpr int TILE_X = 128;
-constexpr int BOX_X = TILE_X + 2;      // elements per TMA box (1040 B, a multiple of 16 B)
-constexpr int ROW_PITCH = 144;         // doubles per staged row: 1152 B keeps every box destination 128-byte aligned
+constexpr int TILE_X = 128;                   // sites per tile = threads per block
+constexpr int BOX_X = TILE_X + 4;             // elements per box row: [x0-2, x0+130)
+constexpr int BOX_Q = 3;                      // populations per box
+constexpr int BOX_DOUBLES = BOX_X * BOX_Q;    // 396 doubles = 3168 B written per copy
+constexpr int BOX_PITCH = 400;                // doubles between box destinations: 3200 B keeps them 128-byte aligned
+constexpr int STAGE_DOUBLES = 9 * BOX_PITCH;  // 28.8 KB
+constexpr int TMA_MIN_NX = 128;
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -52,7 +61,7 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
             : "memory");
     } while (!ok);
 }
-__device__ __forceinline__ void tma_load_row(uint32_t dst, const CUtensorMap* tmap, int x, int y, int z, int q, uint32_t bar)
+__device__ __forceinline__ void tma_load_box(uint32_t dst, const CUtensorMap* tmap, int x, int y, int z, int q, uint32_t bar)
 {
     asm volatile(
         "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
@@ -60,106 +69,147 @@ __device__ __forceinline__ void tma_load_row(uint32_t dst, const CUtensorMap* tm
         : "memory");
 }
 
-// issue the 27 row copies of tile (x0, y, z); one thread
+__device__ __forceinline__ bool elect_one()
+{
+    uint32_t pred;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "elect.sync _|p, 0xffffffff;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(pred));
+    return pred != 0;
+}
+
+// issue the 9 box copies of the tile (x0, y, z); one thread
 template <bool WALLS>
 __device__ __forceinline__ void issue_tile(const CUtensorMap* tmap, uint32_t s_in, uint32_t bar, int x0, int y, int z,
                                            int ny, int nz)
 {
-    mbar_expect_tx(bar, Q * BOX_X * (uint32_t)sizeof(double));
+    mbar_expect_tx(bar, 9u * BOX_DOUBLES * (uint32_t)sizeof(double));
     const int ys[3] = {(y + 1 == ny) ? 0 : y + 1, y, (y == 0) ? ny - 1 : y - 1};     // y - cy, index b = cy + 1
     const int zs[3] = {(z + 1 == nz) ? 0 : z + 1, z, (z == 0) ? nz - 1 : z - 1};
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
+        // with walls the fluid layers are z = 1..nz-2; x - c_q is solid iff (cz=+1 and z==1) or (cz=-1 and z==nz-2):
+        // the population comes back from the site itself as 26-q; the three q' = 26-q of a box are 24-3b-9c + {0,1,2}
         const bool bounce = WALLS && ((c == 2 && z == 1) || (c == 0 && z == nz - 2));
 #pragma unroll
-        for (int b = 0; b < 3; ++b)
-#pragma unroll
-            for (int a = 0; a < 3; ++a) {
-                const int q = a + 3 * b + 9 * c;
-                const uint32_t dst = s_in + (uint32_t)(q * ROW_PITCH * sizeof(double));
-                if (WALLS && bounce) tma_load_row(dst, tmap, x0, y, z, 26 - q, bar);
-                else tma_load_row(dst, tmap, (a == 2) ? x0 - 2 : x0, ys[b], zs[c], q, bar);   // even box start
-            }
+        for (int b = 0; b < 3; ++b) {
+            const uint32_t dst = s_in + (uint32_t)((3 * c + b) * BOX_PITCH * sizeof(double));
+            if (WALLS && bounce) tma_load_box(dst, tmap, x0 - 2, y, z, 24 - 3 * b - 9 * c, bar);
+            else tma_load_box(dst, tmap, x0 - 2, ys[b], zs[c], 3 * b + 9 * c, bar);
+        }
     }
 }
 
+#ifndef RFLBM_TMA_MIN_BLOCKS
+#define RFLBM_TMA_MIN_BLOCKS 4
+#endif
 template <bool WALLS, bool FORCE, bool NOISE>
-__global__ void __launch_bounds__(TILE_X)
+__global__ void __launch_bounds__(TILE_X, RFLBM_TMA_MIN_BLOCKS)
 step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const double* __restrict__ src, double* __restrict__ dst,
                 const __grid_constant__ StepParams<double> P, int rows)
 {
-    __shared__ __align__(128) double s_in[Q][ROW_PITCH];
+    __shared__ __align__(128) double s_stage[STAGE_DOUBLES];
     __shared__ f64x2 s_tab[NOISE ? LOG_TABLE_N + SC_TABLE_N : 1];
     __shared__ __align__(8) unsigned long long s_bar;
 
     const int z = blockIdx.z;
     if (WALLS && (z == 0 || z == P.nz - 1)) return;            // solid layers are never updated
     const int tid = threadIdx.x;
+    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);    // warp-uniform for the compiler too
     const int x0 = blockIdx.x * TILE_X;
     const int y_begin = blockIdx.y * rows;
     const int y_end = min(y_begin + rows, P.ny);
-    const uint32_t bar = smem_u32(&s_bar), in0 = smem_u32(&s_in[0][0]);
+    const uint32_t bar = smem_u32(&s_bar), in0 = smem_u32(&s_stage[0]);
 
-    if (tid == 0) {
+    if (warp == 0 && elect_one()) {
         mbar_init(bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        issue_tile<WALLS>(&tmap_src, in0, bar, x0, y_begin, z, P.ny, P.nz);
     }
-    __syncthreads();
-    if (tid == 0) issue_tile<WALLS>(&tmap_src, in0, bar, x0, y_begin, z, P.ny, P.nz);
     if (NOISE) stage_tables(P.tables, s_tab);                   // ends with __syncthreads()
+    else __syncthreads();                                       // mbarrier init visible to every waiter
 
     const int x = x0 + tid;
     const bool active = x < P.nx;
     const bool wrap_lo = (x == 0), wrap_hi = (x == P.nx - 1);
+    const bool edge_warp = __any_sync(0xffffffffu, wrap_lo || wrap_hi);
     const long long nxy = (long long)P.nx * P.ny;
+    const uint32_t QS32 = (uint32_t)P.QS;                        // QS < 2^32 (rflbm_create)
+    const double* tile = &s_stage[0] + tid;
+    const bool bounce_lo = WALLS && z == 1, bounce_hi = WALLS && z == P.nz - 2;
     uint32_t parity = 0;
 
     for (int y = y_begin; y < y_end; ++y) {
         const long long s = (long long)x + (long long)P.nx * y + nxy * z;
+        // periodic wrap in x: TMA zero-fills these 9 values; fetch them early, use them after the barrier
+        double wv[3][3];
+        if (edge_warp) {                                        // warp-uniform branch: interior warps skip all of this
+            if (wrap_lo || wrap_hi) {
+                const int ysr[3] = {(y + 1 == P.ny) ? 0 : y + 1, y, (y == 0) ? P.ny - 1 : y - 1};
+                const int zsr[3] = {(z + 1 == P.nz) ? 0 : z + 1, z, (z == 0) ? P.nz - 1 : z - 1};
+#pragma unroll
+                for (int c = 0; c < 3; ++c)
+#pragma unroll
+                    for (int b = 0; b < 3; ++b) {
+                        const long long row = (long long)P.nx * ysr[b] + nxy * zsr[c];
+                        // x+1 -> 0 for cx = -1 (a = 0); x-1 -> nx-1 for cx = +1 (a = 2); nx >= 128 here
+                        const long long at = wrap_hi ? (long long)(0 + 3 * b + 9 * c) * P.QS + row
+                                                     : (long long)(2 + 3 * b + 9 * c) * P.QS + row + (P.nx - 1);
+                        wv[c][b] = __ldg(src + at);
+                    }
+            }
+        }
         mbar_wait(bar, parity);
         parity ^= 1u;
         double g[3][3][3];
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
-            // x - cx sits at element tid + 1 of the box for cx != 0; bounced-back rows hold the site itself at tid
-            const bool bounce = WALLS && ((c == 2 && z == 1) || (c == 0 && z == P.nz - 2));
-            const int side = (WALLS && bounce) ? tid : tid + 1;
+            const bool bounce = (c == 2 && bounce_lo) || (c == 0 && bounce_hi);
 #pragma unroll
             for (int b = 0; b < 3; ++b) {
-                g[c][b][0] = s_in[0 + 3 * b + 9 * c][side];
-                g[c][b][1] = s_in[1 + 3 * b + 9 * c][tid];
-                g[c][b][2] = s_in[2 + 3 * b + 9 * c][side];
+                const double* box = tile + (3 * c + b) * BOX_PITCH;
+                if (WALLS && bounce) {       // rows hold q' = 26-q in ascending q': row 2-a, the site itself at tid+2
+                    g[c][b][0] = box[2 * BOX_X + 2];
+                    g[c][b][1] = box[1 * BOX_X + 2];
+                    g[c][b][2] = box[0 * BOX_X + 2];
+                } else {
+                    g[c][b][0] = box[0 * BOX_X + 3];
+                    g[c][b][1] = box[1 * BOX_X + 2];
+                    g[c][b][2] = box[2 * BOX_X + 1];
+                }
             }
         }
-        __syncthreads();                                       // the tile is in registers: the buffer is free
-        if (tid == 0 && y + 1 < y_end) issue_tile<WALLS>(&tmap_src, in0, bar, x0, y + 1, z, P.ny, P.nz);
+        __syncthreads();                                       // the tile is in registers: the stage is free
+        if (warp == 0 && y + 1 < y_end && elect_one()) issue_tile<WALLS>(&tmap_src, in0, bar, x0, y + 1, z, P.ny, P.nz);
 
-        if (wrap_lo || wrap_hi) {                              // periodic wrap in x: TMA zero-filled these
-            const int ysr[3] = {(y + 1 == P.ny) ? 0 : y + 1, y, (y == 0) ? P.ny - 1 : y - 1};
-            const int zsr[3] = {(z + 1 == P.nz) ? 0 : z + 1, z, (z == 0) ? P.nz - 1 : z - 1};
+        if (edge_warp) {
+            if (wrap_lo || wrap_hi) {
 #pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                const bool bounce = WALLS && ((c == 2 && z == 1) || (c == 0 && z == P.nz - 2));
-                if (bounce) continue;                          // bounced populations come from the site itself
+                for (int c = 0; c < 3; ++c) {
+                    const bool bounce = (c == 2 && bounce_lo) || (c == 0 && bounce_hi);
+                    if (WALLS && bounce) continue;             // bounced populations come from the site itself
 #pragma unroll
-                for (int b = 0; b < 3; ++b) {
-                    const long long row = (long long)P.nx * ysr[b] + nxy * zsr[c];
-                    if (wrap_hi) g[c][b][0] = __ldg(src + (long long)(0 + 3 * b + 9 * c) * P.N + row);                // x+1 -> 0
-                    if (wrap_lo) g[c][b][2] = __ldg(src + (long long)(2 + 3 * b + 9 * c) * P.N + row + (P.nx - 1));   // x-1 -> nx-1
+                    for (int b = 0; b < 3; ++b) {
+                        if (wrap_hi) g[c][b][0] = wv[c][b];
+                        else g[c][b][2] = wv[c][b];
+                    }
                 }
             }
         }
         if (active) {
             collide<double, FORCE, NOISE>(g, P, (uint32_t)s, s_tab, s_tab + LOG_TABLE_N);
             char* out = reinterpret_cast<char*>(dst + s);
-            const long long qstride = P.N * (long long)sizeof(double);
 #pragma unroll
             for (int c = 0; c < 3; ++c)
 #pragma unroll
                 for (int b = 0; b < 3; ++b)
 #pragma unroll
-                    for (int a = 0; a < 3; ++a)
-                        __stcs(reinterpret_cast<double*>(out + (long long)(a + 3 * b + 9 * c) * qstride), g[c][b][a]);
+                    for (int a = 0; a < 3; ++a) {
+                        const unsigned long long off = (unsigned long long)QS32 * (unsigned)(8 * (a + 3 * b + 9 * c));
+                        __stcs(reinterpret_cast<double*>(out + off), g[c][b][a]);
+                    }
         }
     }
 }
