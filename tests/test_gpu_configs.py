@@ -1,0 +1,177 @@
+"""GPU runs of BASELINE.json configs[1..4] through the C-ABI (configs[0] is tests/test_gpu_parity.py).
+
+configs[1] 64^3 equipartition + flat structure factor, configs[2] 256^3 Taylor-Green decay, configs[3] 512^3 in the
+launch configuration bench.py times (TMA kernel): sampled outputs against the oracle's single-site collision plus
+conservation, configs[4] 256^3 fp32 channel against the start-up series of the oracle pin P12.
+Statistics are computed test-side (numpy / torch on the downloaded moments); the expected values are the closed
+forms that also pin the oracle."""
+import numpy as np
+import pytest
+
+import oracle
+from analysis import fit_decay_rate, shell_spectrum
+from paper_2507_08820_b200 import binding, synthetic
+
+pytestmark = pytest.mark.gpu
+
+
+def torch_():
+    import torch
+    return torch
+
+
+@pytest.mark.parametrize("tau", [0.6, 1.0])
+def test_config2_equipartition_and_structure_factor_64(tau):
+    """<u_a^2> rho0/kT = 1 +- 0.005 and S_rho(k), S_j(k) = 1 shell by shell within 4 sigma + 0.5 % (R11, P10), where
+    sigma = 1/sqrt(n_eff cnt/2): |X_k|^2 of a complex Gaussian mode has relative spread 1, k and -k are the same
+    mode, and of the 91 snapshots taken 20 steps apart only n_eff = min(91, 1800 nu k^2) are independent (the
+    variance of a mode decorrelates at rate 2 nu k^2).  That is +-1.5 % on the well-populated shells.
+    The run starts cold (no fluctuations), so a mode of wavenumber k reaches its stationary variance as
+    1 - exp(-2 nu k^2 t); averaged over the sampling window [200, 2000] that leaves a deficit of
+    exp(-2 nu k^2 200) / (2 nu k^2 1800).  Shells where this exceeds 0.2 % (|k| L/2pi < 5 at tau=0.6, < 3 at
+    tau=1.0) are reported only: they are slow, not wrong (measured: 0.96 and 0.98 on shells 3, 4 at tau=0.6)."""
+    n, kT, rho0 = 64, 1e-4, 1.0
+    sim = binding.Rflbm(n, n, n, tau, kT, rho0, 7)
+    sim.init()
+    sim.step(200)
+    u2, acc, cnt = [], {}, None
+    while sim.step_count <= 2000:
+        rho, u = sim.moments()
+        rho, u = rho.cpu().numpy(), u.cpu().numpy()
+        u2.append((u ** 2).mean(axis=(1, 2, 3)))
+        for name, fld, norm in [("rho", rho, 3 * rho0 * kT)] + [(f"j{a}", rho * u[a], rho0 * kT) for a in range(3)]:
+            tot, cnt = shell_spectrum(fld)
+            acc.setdefault(name, []).append(tot / norm)
+        sim.step(20)
+    u2 = np.mean(u2, axis=0) * rho0 / kT
+    assert np.abs(u2 - 1.0).max() < 0.005, u2
+    nu = (tau - 0.5) / 3.0
+    shells = np.arange(len(cnt))
+    k2 = (2 * np.pi * shells / n) ** 2
+    rate = np.maximum(2 * nu * k2, 1e-300)
+    gate = (np.exp(-rate * 200) / (rate * 1800) < 0.002) & (cnt >= 30) & (shells >= 1)
+    assert gate.sum() >= 40 and gate[5:30].all()
+    for name in ("rho", "j0", "j1", "j2"):
+        s = np.mean(acc[name], axis=0)
+        assert abs(s[1:].sum() / cnt[1:].sum() - 1.0) < 0.005, name
+        sk = s[gate] / cnt[gate]
+        n_eff = np.minimum(len(acc[name]), 1800 * nu * k2[gate])
+        tol = 4.0 / np.sqrt(n_eff * cnt[gate] / 2.0) + 0.005
+        assert (np.abs(sk - 1.0) < tol).all(), (name, tau, np.abs(sk - 1.0) / tol)
+        assert tol[20:40].max() < 0.02
+    d = sim.diagnostics()
+    assert abs(d[0] / n ** 3 - rho0) < 1e-12 and max(abs(v) for v in d[1:4]) / n ** 3 < 1e-14
+
+
+@pytest.mark.parametrize("tau,kT,tol", [(0.51, 0.0, 0.03), (0.8, 0.0, 0.005), (1.5, 0.0, 0.005),
+                                        (0.51, 1e-5, 0.25), (0.8, 1e-5, 0.02), (1.5, 1e-5, 0.02)])
+def test_config3_taylor_green_decay_256(tau, kT, tol):
+    """Decay rate of the R15 vortex = 2 nu k^2, nu = (tau - 1/2)/3, with and without thermal noise.
+    tau = 0.51: the amplitude decays by only 0.16 % over the fit window, and the weak sound wave radiated by the
+    uniform-density start (R15: an O(u0^2) = 1e-4 pressure mismatch, one acoustic period = 443 steps, barely damped
+    at this viscosity) modulates it at the 1e-5 level: 3 % on the rate without noise (measured 1.8 %), 25 % with."""
+    torch = torch_()
+    n, nz = 256, 256
+    sim = binding.Rflbm(n, n, nz, tau, kT, 1.0, 3)
+    rho0, u0 = synthetic.taylor_green_fields(n, n, nz, u0=0.01)
+    sim.init(torch.from_numpy(rho0), torch.from_numpy(u0))
+    x = torch.arange(n, device="cuda", dtype=torch.float64)
+    shape = (torch.sin(2 * np.pi * x / n)[None, None, :] * torch.cos(2 * np.pi * x / n)[None, :, None])
+    rho = torch.empty((nz, n, n), dtype=torch.float64, device="cuda")
+    u = torch.empty((3, nz, n, n), dtype=torch.float64, device="cuda")
+    sim.step(100)
+    ts, amps = [], []
+    while sim.step_count <= 500:
+        sim.moments(rho, u)
+        ts.append(sim.step_count)
+        amps.append(4.0 * float((u[0] * shape).mean()))
+        sim.step(10)
+    k2 = 2 * (2 * np.pi / n) ** 2
+    nu = (tau - 0.5) / 3.0
+    assert abs(fit_decay_rate(ts, amps) / (nu * k2) - 1.0) < tol, (fit_decay_rate(ts, amps), nu * k2)
+
+
+def test_config4_sampled_parity_and_conservation_512():
+    """512^3 fp64 through the TMA kernel (the bench configuration): one step of sampled sites against the oracle's
+    single-site collision (exact neighbours through the periodic wrap), then conservation over the run."""
+    torch = torch_()
+    n, tau, kT, seed = 512, 0.8, 1e-4, 11
+    free, _ = torch.cuda.mem_get_info()
+    if free < 125e9:
+        pytest.skip("needs 125 GB of free device memory")
+    sim = binding.Rflbm(n, n, n, tau, kT, 1.0, seed)
+    sim.set_kernel_variant(binding.KERNEL_TMA)
+    sim.init()
+    sim.step(3)                                                # a thermal, site-dependent state
+    f0 = sim.get_populations()
+    sim.step(1)
+    f1 = sim.get_populations()
+    c = oracle.tables()[0]
+    rng = np.random.default_rng(5)
+    pts = rng.integers(0, n, size=(160, 3)).tolist()
+    edge = [0, 1, 126, 127, 128, 129, 255, 256, 510, 511]      # tile boundaries of the TMA kernel and the wrap
+    pts += [(x, int(rng.integers(0, n)), int(rng.integers(0, n))) for x in edge]
+    pts += [(int(rng.integers(0, n)), y, z) for y in (0, 15, 16, 511) for z in (0, 511, 200)]
+    pts += [(0, 0, 0), (511, 511, 511), (0, 511, 0), (511, 0, 511)]
+    P = torch.tensor(pts, device="cuda")
+    g_all = f0[:, P[:, 2], P[:, 1], P[:, 0]].T.cpu().numpy()   # [npts, 27]
+    got = torch.empty((len(pts), 27), dtype=torch.float64, device="cuda")
+    for i in range(27):
+        xs, ys, zs = (P[:, 0] + int(c[i][0])) % n, (P[:, 1] + int(c[i][1])) % n, (P[:, 2] + int(c[i][2])) % n
+        got[:, i] = f1[i, zs, ys, xs]
+    got = got.cpu().numpy()
+    worst = 0.0
+    for k, (x, y, z) in enumerate(pts):
+        want = oracle.collide_site(g_all[k], tau, kT, seed, site=x + n * (y + n * z), t=3)
+        worst = max(worst, float(np.abs(got[k] - want).max()))
+    assert worst < 1e-13, worst
+    del f0, f1
+    d0 = sim.diagnostics()
+    sim.step(20)
+    d1 = sim.diagnostics()
+    N = n ** 3
+    assert abs(d1[0] - d0[0]) / N < 1e-13 and abs(d0[0] / N - 1.0) < 1e-12
+    assert max(abs(v) for v in d1[1:4]) / N < 1e-14
+    assert np.abs(np.array(d1[7:10]) / kT - 1.0).max() < 0.01   # <u_a^2> = kT/rho0 (thermalised within ~10 steps)
+
+
+def test_config5_channel_fp32_startup_profile_256():
+    """256^3 channel, fp32 storage, walls z=0,255, g_x=1e-6, tau=0.9, kT=1e-4, 5000 steps: the plane-averaged
+    u_x(z) follows the start-up series of P12 (5000 steps = 1 % of H^2/nu: a plug with boundary layers), and the
+    bulk velocity variance is kT/rho0.  Near-wall variance is reported, not gated (parity unpinned)."""
+    n, nz, tau, g, kT = 256, 256, 0.9, 1e-6, 1e-4
+    sim = binding.Rflbm(n, n, nz, tau, kT, 1.0, 5, binding.F32)
+    sim.set_walls_z(True)
+    sim.set_force(g, 0.0, 0.0)
+    sim.init()
+    d0 = sim.diagnostics()
+    sim.step(4000)
+    prof, var, ts = [], [], []
+    while sim.step_count <= 5000:
+        rho, u = sim.moments()
+        ud = u.double()
+        prof.append(ud[0].mean(dim=(1, 2)).cpu().numpy())
+        var.append(((ud - ud.mean(dim=(2, 3), keepdim=True)) ** 2).mean(dim=(2, 3)).cpu().numpy())
+        ts.append(sim.step_count)
+        sim.step(100)
+    H = nz - 2
+    nu = (tau - 0.5) / 3.0
+    z = np.arange(1, nz - 1)
+    lam = (tau - 0.5) / 2.0
+
+    def series(t):
+        steady = g / (2 * nu) * ((z - 0.5) * (nz - 1.5 - z) + 4 * lam / 3 - 0.25)
+        ser = sum(4 * g * H ** 2 / (nu * np.pi ** 3 * m ** 3) * np.sin(m * np.pi * (z - 0.5) / H)
+                  * np.exp(-m ** 2 * np.pi ** 2 * nu * t / H ** 2) for m in range(1, 4000, 2))
+        return steady - ser
+
+    want = np.mean([series(t) for t in ts], axis=0)
+    got = np.mean(prof, axis=0)[1:-1]
+    umax = want.max()
+    assert 4.0e-3 < umax < 5.0e-3                                   # ~ g t: still a plug
+    assert np.abs(got - want).max() < 0.03 * umax, np.abs(got - want).max() / umax
+    v = np.mean(var, axis=0)[:, 1:-1] / kT                           # [3, fluid layers]
+    assert np.abs(v[:, 20:-20].mean(axis=1) - 1.0).max() < 0.02, v[:, 20:-20].mean(axis=1)
+    print("near-wall <du^2>/kT (layers 1..3):", v[:, :3])
+    d1 = sim.diagnostics()
+    assert abs(d1[0] / d0[0] - 1.0) < 1e-5                           # fp32 storage: mass drift reported and bounded
