@@ -73,7 +73,7 @@ int rflbm_init(rflbm_t* h, const void* rho_dev, const void* u_dev);
 int rflbm_step(rflbm_t* h, int nsteps);
 
 /* Which implementation of the step kernel rflbm_step launches.  AUTO (default): the TMA-staged kernel when the
- * lattice allows it (fp64, nx >= 128, nx even), else the plain one-thread-per-site kernel.  PLAIN forces the
+ * lattice allows it (nx >= 128 and nx*sizeof(real) a multiple of 16), else the plain one-thread-per-site kernel.  PLAIN forces the
  * latter; TMA fails with EINVAL at rflbm_step if the lattice does not allow it.  All variants compute the same
  * update (same results up to the bit: identical arithmetic, only the data movement differs). */
 enum { RFLBM_KERNEL_AUTO = 0, RFLBM_KERNEL_PLAIN = 1, RFLBM_KERNEL_TMA = 2 };

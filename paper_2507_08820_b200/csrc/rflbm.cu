@@ -79,7 +79,7 @@ typedef CUresult (*encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_
                                     const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                     CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-// 4-D view [27][nz][ny][nx] of one fp64 population buffer, box = BOX_X consecutive x of one row of BOX_Q arrays
+// 4-D view [27][nz][ny][nx] of one population buffer, box = BOX_X consecutive x of one row of BOX_Q arrays
 static bool make_tensor_map(rflbm* h, void* base, CUtensorMap* out)
 {
     void* fn = nullptr;
@@ -90,10 +90,12 @@ static bool make_tensor_map(rflbm* h, void* base, CUtensorMap* out)
         return false;
     }
     const cuuint64_t dims[4] = {(cuuint64_t)h->nx, (cuuint64_t)h->ny, (cuuint64_t)h->nz, (cuuint64_t)Q};
-    const cuuint64_t strides[3] = {(cuuint64_t)h->nx * 8, (cuuint64_t)h->nx * h->ny * 8, (cuuint64_t)h->QS * 8};
-    const cuuint32_t box[4] = {BOX_X, 1, 1, BOX_Q};   // 132 x 3 elements: 16-byte aligned starts, see rflbm_step_tma.cuh
+    const bool f64 = h->precision == RFLBM_F64;
+    const cuuint64_t es = f64 ? 8 : 4;
+    const cuuint64_t strides[3] = {(cuuint64_t)h->nx * es, (cuuint64_t)h->nx * h->ny * es, (cuuint64_t)h->QS * es};
+    const cuuint32_t box[4] = {(cuuint32_t)(f64 ? TmaGeom<double>::BOX_X : TmaGeom<float>::BOX_X), 1, 1, BOX_Q};   // 16-byte aligned starts
     const cuuint32_t estr[4] = {1, 1, 1, 1};
-    const CUresult r = ((encode_tiled_fn)fn)(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box, estr,
+    const CUresult r = ((encode_tiled_fn)fn)(out, f64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, base, dims, strides, box, estr,
                                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                                              CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS;
@@ -168,9 +170,9 @@ extern "C" int rflbm_set_workspace(rflbm_t* h, void* dev_ptr, size_t bytes)
     fill_normal_tables(host_tab, host_tab + LOG_TABLE_N);
     const int rc = check_cuda(h, cudaMemcpy(h->tables, host_tab, TABLE_BYTES, cudaMemcpyHostToDevice), "table upload");
     if (rc != RFLBM_OK) return rc;
-    // TMA path: fp64, rows of at least one 128-site tile, row pitch a multiple of 16 bytes
+    // TMA path: rows of at least one 128-site tile, row pitch a multiple of 16 bytes (nx even for fp64, nx % 4 == 0 for fp32)
     h->tma_ok = false;
-    if (h->precision == RFLBM_F64 && h->nx >= TMA_MIN_NX && h->nx % 2 == 0)
+    if (h->nx >= TMA_MIN_NX && h->nx % (16 / (int)real_size(h)) == 0)
         h->tma_ok = make_tensor_map(h, h->buf[0], &h->tmap[0]) && make_tensor_map(h, h->buf[1], &h->tmap[1]);
     return RFLBM_OK;
 }
@@ -313,30 +315,28 @@ static void launch_step(rflbm* h, const StepParams<real>& P)
         <<<h->grid, h->block, 0, h->stream>>>((const real*)h->buf[h->cur], (real*)h->buf[h->cur ^ 1], P);
 }
 
-template <bool WALLS, bool FORCE, bool NOISE>
-static void launch_step_tma(rflbm* h, const StepParams<double>& P)
+template <typename real, bool WALLS, bool FORCE, bool NOISE>
+static void launch_step_tma(rflbm* h, const StepParams<real>& P)
 {
     const dim3 grid((h->nx + TILE_X - 1) / TILE_X, (h->ny + h->tma_rows - 1) / h->tma_rows, h->nz);
-    step_kernel_tma<WALLS, FORCE, NOISE><<<grid, TILE_X, 0, h->stream>>>(
-        h->tmap[h->cur], (const double*)h->buf[h->cur], (double*)h->buf[h->cur ^ 1], P, h->tma_rows);
+    step_kernel_tma<real, WALLS, FORCE, NOISE><<<grid, TILE_X, 0, h->stream>>>(
+        h->tmap[h->cur], (const real*)h->buf[h->cur], (real*)h->buf[h->cur ^ 1], P, h->tma_rows);
 }
 
 static bool use_tma(const rflbm* h) { return h->tma_ok && h->variant != RFLBM_KERNEL_PLAIN; }
 
 template <typename real>
-static void dispatch_tma(rflbm*, const StepParams<real>&, int) {}
-template <>
-void dispatch_tma<double>(rflbm* h, const StepParams<double>& P, int variant)
+static void dispatch_tma(rflbm* h, const StepParams<real>& P, int variant)
 {
     switch (variant) {
-        case 0: launch_step_tma<false, false, false>(h, P); break;
-        case 1: launch_step_tma<false, false, true>(h, P); break;
-        case 2: launch_step_tma<false, true, false>(h, P); break;
-        case 3: launch_step_tma<false, true, true>(h, P); break;
-        case 4: launch_step_tma<true, false, false>(h, P); break;
-        case 5: launch_step_tma<true, false, true>(h, P); break;
-        case 6: launch_step_tma<true, true, false>(h, P); break;
-        default: launch_step_tma<true, true, true>(h, P); break;
+        case 0: launch_step_tma<real, false, false, false>(h, P); break;
+        case 1: launch_step_tma<real, false, false, true>(h, P); break;
+        case 2: launch_step_tma<real, false, true, false>(h, P); break;
+        case 3: launch_step_tma<real, false, true, true>(h, P); break;
+        case 4: launch_step_tma<real, true, false, false>(h, P); break;
+        case 5: launch_step_tma<real, true, false, true>(h, P); break;
+        case 6: launch_step_tma<real, true, true, false>(h, P); break;
+        default: launch_step_tma<real, true, true, true>(h, P); break;
     }
 }
 
@@ -345,7 +345,7 @@ static int do_step(rflbm* h, int nsteps)
 {
     const bool noise = h->kT > 0.0;       // kT = 0: deterministic Reg-LBM, RNG skipped entirely (R17)
     if (h->variant == RFLBM_KERNEL_TMA && !h->tma_ok)
-        return fail(h, RFLBM_EINVAL, "TMA kernel needs fp64, nx >= 128 and nx even");
+        return fail(h, RFLBM_EINVAL, "TMA kernel needs nx >= 128 and a row pitch that is a multiple of 16 bytes");
     for (int s = 0; s < nsteps; ++s) {
         const StepParams<real> P = step_params<real>(h, h->t);
         const int variant = (h->walls ? 4 : 0) | (h->force ? 2 : 0) | (noise ? 1 : 0);

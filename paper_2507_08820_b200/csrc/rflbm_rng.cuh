@@ -127,16 +127,33 @@ __device__ __forceinline__ void normal_pair(uint32_t xa, uint32_t xb, const f64x
     normal_pair_fast(xa, xb, lg, sc, z0, z1);
 }
 
-// fp32 mode (R14): 24-bit uniforms ((x>>8)+0.5)/2^24, float arithmetic, accurate (non fast-math) functions.
+// fp32 mode (R14): 24-bit uniforms ((x>>8)+0.5)/2^24, float arithmetic on the special-function unit.
+// The fp32 path owes the oracle 1e-5 on the populations (BASELINE.json), i.e. ~1e-4 on a normal; the hardware
+// approximations are far inside that and keep the fp32 kernel on the HBM roofline (the accurate logf / sqrtf /
+// sincospif cost ~45 instructions per pair and halved the throughput, profiles/r01d):
+//   -2 ln u = (-2 ln 2) lg2.approx(u)   (MUFU.LG2, abs. error < 2^-22 on lg2, u in [2^-25, 1))
+//   (for u within 2^-10 of 1 the series 2v + v^2 of -2 ln(1-v), v = 1-u exact, replaces it: R error < 1e-5 everywhere)
+//   R = W rsqrt.approx(W)                (MUFU.RSQ, 2 ulp; W >= 5.9e-8 > 0)
+//   sin, cos(2 pi u) = -sin, -cos(2 pi u - pi), argument in (-pi, pi) where MUFU.SIN/COS are good to 2^-21.4
 __device__ __forceinline__ void normal_pair(uint32_t xa, uint32_t xb, const f64x2*, const f64x2*, float& z0, float& z1)
 {
-    const float ua = ((float)(xa >> 8) + 0.5f) * (1.0f / 16777216.0f);
-    const float two_ub = ((float)(xb >> 8) + 0.5f) * (1.0f / 8388608.0f);
-    const float R = sqrtf(-2.0f * logf(ua));
+    const uint32_t k = xa >> 8;
+    const float ua = ((float)k + 0.5f) * (1.0f / 16777216.0f);     // rounds to 1.0f for the last k: handled below
+    float l2, rs;
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(l2) : "f"(ua));        // ua is a normal number: no denormal scaling needed
+    float W = -1.3862943611198906f * l2;
+    if (k >= 16777216u - 16384u) {                                  // u within 2^-10 of 1 (3 % of the warps): the
+        const float v = ((float)(16777216u - k) - 0.5f) * (1.0f / 16777216.0f);   // absolute error of lg2 would show,
+        W = fmaf(v, v, 2.0f * v);                                   // so -2 ln(1-v) = 2v + v^2 + O(v^3 < 1e-9), v exact
+    }
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(rs) : "f"(W));
+    const float R = W * rs;
+    // 2 pi u - pi = 2 pi ((xb>>8) - 2^23 + 0.5) / 2^24, exact integer part
+    const float th = ((float)((int)(xb >> 8) - 8388608) + 0.5f) * (6.283185307179586f / 16777216.0f);
     float s, c;
-    sincospif(two_ub, &s, &c);
-    z0 = R * c;
-    z1 = R * s;
+    __sincosf(th, &s, &c);
+    z0 = -R * c;
+    z1 = -R * s;
 }
 
 }  // namespace rflbm_dev

@@ -30,12 +30,17 @@
 namespace rflbm_dev {
 
 constexpr int TILE_X = 128;                   // sites per tile = threads per block
-constexpr int BOX_X = TILE_X + 4;             // elements per box row: [x0-2, x0+130)
 constexpr int BOX_Q = 3;                      // populations per box
-constexpr int BOX_DOUBLES = BOX_X * BOX_Q;    // 396 doubles = 3168 B written per copy
-constexpr int BOX_PITCH = 400;                // doubles between box destinations: 3200 B keeps them 128-byte aligned
-constexpr int STAGE_DOUBLES = 9 * BOX_PITCH;  // 28.8 KB
 constexpr int TMA_MIN_NX = 128;
+// per element type: 16-byte halo on each side of the tile (2 doubles / 4 floats), box = [x0-HALO, x0+128+HALO)
+template <typename real> struct TmaGeom {
+    static constexpr int HALO = 16 / (int)sizeof(real);
+    static constexpr int BOX_X = TILE_X + 2 * HALO;                                  // 132 doubles / 136 floats
+    static constexpr int BOX_BYTES = BOX_X * BOX_Q * (int)sizeof(real);              // 3168 B / 1632 B per copy
+    static constexpr int BOX_PITCH_BYTES = (BOX_BYTES + 127) / 128 * 128;            // destinations stay 128-byte aligned
+    static constexpr int BOX_PITCH = BOX_PITCH_BYTES / (int)sizeof(real);            // in elements
+    static constexpr int STAGE_BYTES = 9 * BOX_PITCH_BYTES;                          // 28.8 KB / 15.0 KB
+};
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -81,11 +86,12 @@ __device__ __forceinline__ bool elect_one()
 }
 
 // issue the 9 box copies of the tile (x0, y, z); one thread
-template <bool WALLS>
+template <typename real, bool WALLS>
 __device__ __forceinline__ void issue_tile(const CUtensorMap* tmap, uint32_t s_in, uint32_t bar, int x0, int y, int z,
                                            int ny, int nz)
 {
-    mbar_expect_tx(bar, 9u * BOX_DOUBLES * (uint32_t)sizeof(double));
+    using G = TmaGeom<real>;
+    mbar_expect_tx(bar, 9u * (uint32_t)G::BOX_BYTES);
     const int ys[3] = {(y + 1 == ny) ? 0 : y + 1, y, (y == 0) ? ny - 1 : y - 1};     // y - cy, index b = cy + 1
     const int zs[3] = {(z + 1 == nz) ? 0 : z + 1, z, (z == 0) ? nz - 1 : z - 1};
 #pragma unroll
@@ -95,23 +101,23 @@ __device__ __forceinline__ void issue_tile(const CUtensorMap* tmap, uint32_t s_i
         const bool bounce = WALLS && ((c == 2 && z == 1) || (c == 0 && z == nz - 2));
 #pragma unroll
         for (int b = 0; b < 3; ++b) {
-            const uint32_t dst = s_in + (uint32_t)((3 * c + b) * BOX_PITCH * sizeof(double));
-            if (WALLS && bounce) tma_load_box(dst, tmap, x0 - 2, y, z, 24 - 3 * b - 9 * c, bar);
-            else tma_load_box(dst, tmap, x0 - 2, ys[b], zs[c], 3 * b + 9 * c, bar);
+            const uint32_t dst = s_in + (uint32_t)((3 * c + b) * G::BOX_PITCH_BYTES);
+            if (WALLS && bounce) tma_load_box(dst, tmap, x0 - G::HALO, y, z, 24 - 3 * b - 9 * c, bar);
+            else tma_load_box(dst, tmap, x0 - G::HALO, ys[b], zs[c], 3 * b + 9 * c, bar);
         }
     }
 }
 
-#ifndef RFLBM_TMA_MIN_BLOCKS
-#define RFLBM_TMA_MIN_BLOCKS 4
-#endif
-template <bool WALLS, bool FORCE, bool NOISE>
-__global__ void __launch_bounds__(TILE_X, RFLBM_TMA_MIN_BLOCKS)
-step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const double* __restrict__ src, double* __restrict__ dst,
-                const __grid_constant__ StepParams<double> P, int rows)
+// fp64: 128 registers, 41 KB -> 4 blocks per SM; fp32: 64 registers, 15 KB -> 8 blocks per SM
+template <typename real, bool WALLS, bool FORCE, bool NOISE>
+__global__ void __launch_bounds__(TILE_X, sizeof(real) == 8 ? 4 : 8)
+step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const real* __restrict__ src, real* __restrict__ dst,
+                const __grid_constant__ StepParams<real> P, int rows)
 {
-    __shared__ __align__(128) double s_stage[STAGE_DOUBLES];
-    __shared__ f64x2 s_tab[NOISE ? LOG_TABLE_N + SC_TABLE_N : 1];
+    using G = TmaGeom<real>;
+    constexpr bool TABLES = NOISE && sizeof(real) == 8;         // the fp32 Box-Muller needs no tables
+    __shared__ __align__(128) real s_stage[G::STAGE_BYTES / sizeof(real)];
+    __shared__ f64x2 s_tab[TABLES ? LOG_TABLE_N + SC_TABLE_N : 1];
     __shared__ __align__(8) unsigned long long s_bar;
 
     const int z = blockIdx.z;
@@ -126,9 +132,9 @@ step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const double* __re
     if (warp == 0 && elect_one()) {
         mbar_init(bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        issue_tile<WALLS>(&tmap_src, in0, bar, x0, y_begin, z, P.ny, P.nz);
+        issue_tile<real, WALLS>(&tmap_src, in0, bar, x0, y_begin, z, P.ny, P.nz);
     }
-    if (NOISE) stage_tables(P.tables, s_tab);                   // ends with __syncthreads()
+    if (TABLES) stage_tables(P.tables, s_tab);                  // ends with __syncthreads()
     else __syncthreads();                                       // mbarrier init visible to every waiter
 
     const int x = x0 + tid;
@@ -137,14 +143,14 @@ step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const double* __re
     const bool edge_warp = __any_sync(0xffffffffu, wrap_lo || wrap_hi);
     const long long nxy = (long long)P.nx * P.ny;
     const uint32_t QS32 = (uint32_t)P.QS;                        // QS < 2^32 (rflbm_create)
-    const double* tile = &s_stage[0] + tid;
+    const real* tile = &s_stage[0] + tid;
     const bool bounce_lo = WALLS && z == 1, bounce_hi = WALLS && z == P.nz - 2;
     uint32_t parity = 0;
 
     for (int y = y_begin; y < y_end; ++y) {
         const long long s = (long long)x + (long long)P.nx * y + nxy * z;
         // periodic wrap in x: TMA zero-fills these 9 values; fetch them early, use them after the barrier
-        double wv[3][3];
+        real wv[3][3];
         if (edge_warp) {                                        // warp-uniform branch: interior warps skip all of this
             if (wrap_lo || wrap_hi) {
                 const int ysr[3] = {(y + 1 == P.ny) ? 0 : y + 1, y, (y == 0) ? P.ny - 1 : y - 1};
@@ -163,26 +169,26 @@ step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const double* __re
         }
         mbar_wait(bar, parity);
         parity ^= 1u;
-        double g[3][3][3];
+        real g[3][3][3];
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
             const bool bounce = (c == 2 && bounce_lo) || (c == 0 && bounce_hi);
 #pragma unroll
             for (int b = 0; b < 3; ++b) {
-                const double* box = tile + (3 * c + b) * BOX_PITCH;
-                if (WALLS && bounce) {       // rows hold q' = 26-q in ascending q': row 2-a, the site itself at tid+2
-                    g[c][b][0] = box[2 * BOX_X + 2];
-                    g[c][b][1] = box[1 * BOX_X + 2];
-                    g[c][b][2] = box[0 * BOX_X + 2];
+                const real* box = tile + (3 * c + b) * G::BOX_PITCH;
+                if (WALLS && bounce) {       // rows hold q' = 26-q in ascending q': row 2-a, the site itself at tid+HALO
+                    g[c][b][0] = box[2 * G::BOX_X + G::HALO];
+                    g[c][b][1] = box[1 * G::BOX_X + G::HALO];
+                    g[c][b][2] = box[0 * G::BOX_X + G::HALO];
                 } else {
-                    g[c][b][0] = box[0 * BOX_X + 3];
-                    g[c][b][1] = box[1 * BOX_X + 2];
-                    g[c][b][2] = box[2 * BOX_X + 1];
+                    g[c][b][0] = box[0 * G::BOX_X + G::HALO + 1];
+                    g[c][b][1] = box[1 * G::BOX_X + G::HALO];
+                    g[c][b][2] = box[2 * G::BOX_X + G::HALO - 1];
                 }
             }
         }
         __syncthreads();                                       // the tile is in registers: the stage is free
-        if (warp == 0 && y + 1 < y_end && elect_one()) issue_tile<WALLS>(&tmap_src, in0, bar, x0, y + 1, z, P.ny, P.nz);
+        if (warp == 0 && y + 1 < y_end && elect_one()) issue_tile<real, WALLS>(&tmap_src, in0, bar, x0, y + 1, z, P.ny, P.nz);
 
         if (edge_warp) {
             if (wrap_lo || wrap_hi) {
@@ -199,16 +205,18 @@ step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const double* __re
             }
         }
         if (active) {
-            collide<double, FORCE, NOISE>(g, P, (uint32_t)s, s_tab, s_tab + LOG_TABLE_N);
-            char* out = reinterpret_cast<char*>(dst + s);
+            collide<real, FORCE, NOISE>(g, P, (uint32_t)s, s_tab, s_tab + LOG_TABLE_N);
+            const unsigned long long out = reinterpret_cast<unsigned long long>(dst + s);
 #pragma unroll
             for (int c = 0; c < 3; ++c)
 #pragma unroll
                 for (int b = 0; b < 3; ++b)
 #pragma unroll
                     for (int a = 0; a < 3; ++a) {
-                        const unsigned long long off = (unsigned long long)QS32 * (unsigned)(8 * (a + 3 * b + 9 * c));
-                        __stcs(reinterpret_cast<double*>(out + off), g[c][b][a]);
+                        // one IMAD.WIDE.U32 per store: out + QS * sizeof(real) * q (QS < 2^32, so the 32x32->64 product is exact)
+                        unsigned long long at;
+                        asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(at) : "r"(QS32), "r"((unsigned)sizeof(real) * (a + 3 * b + 9 * c)), "l"(out));
+                        __stcs(reinterpret_cast<real*>(at), g[c][b][a]);
                     }
         }
     }

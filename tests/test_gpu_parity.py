@@ -212,7 +212,33 @@ def test_tma_kernel_matches_plain_kernel_and_oracle(shape, walls, force, kT):
     assert np.abs(outs[binding.KERNEL_TMA].cpu().numpy() - ref.get_populations()).max() < TOL64
 
 
+@pytest.mark.parametrize("shape,walls,force,kT", [((128, 5, 4), False, None, 1e-4), ((260, 18, 5), True, (1e-5, 2e-6, -3e-6), 1e-4),
+                                                 ((384, 3, 3), False, (1e-6, 0.0, 0.0), 0.0)])
+def test_tma_kernel_fp32_matches_plain_kernel_and_oracle(shape, walls, force, kT):
+    """fp32 instantiation of the TMA kernel (nx >= 128, nx % 4 == 0): 136-float boxes, 4-element halo."""
+    torch = torch_()
+    nx, ny, nz = shape
+    fields = synthetic.smooth_random_fields(nx, ny, nz, 14)
+    outs = {}
+    for variant in (binding.KERNEL_TMA, binding.KERNEL_PLAIN):
+        sim, ref = make_pair(nx, ny, nz, 0.8, kT, 19, precision=binding.F32, walls=walls, force=force)
+        sim.set_kernel_variant(variant)
+        init_pair(sim, ref, fields)
+        sim.step(40)
+        outs[variant] = sim.get_populations()
+    ref.step(40)
+    assert torch.equal(outs[binding.KERNEL_TMA], outs[binding.KERNEL_PLAIN])
+    assert np.abs(outs[binding.KERNEL_TMA].cpu().numpy().astype(np.float64) - ref.get_populations()).max() < TOL32
+
+
 def test_tma_variant_rejected_when_lattice_does_not_allow_it():
+    for nx, prec in ((33, binding.F64), (130, binding.F32)):     # too short; row pitch 520 B not a multiple of 16
+        sim = binding.Rflbm(nx, 4, 4, 0.8, 1e-4, precision=prec)
+        sim.set_kernel_variant(binding.KERNEL_TMA)
+        sim.init()
+        with pytest.raises(binding.RflbmError) as e:
+            sim.step(1)
+        assert e.value.code == binding.EINVAL
     sim = binding.Rflbm(33, 4, 4, 0.8, 1e-4)
     sim.set_kernel_variant(binding.KERNEL_TMA)
     sim.init()
