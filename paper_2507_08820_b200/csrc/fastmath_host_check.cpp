@@ -31,7 +31,7 @@ void fm_sqrt(const double* w, double* out, long n)
 void fm_sincos(const uint32_t* x, double* s, double* c, long n)
 {
     ready();
-    for (long i = 0; i < n; ++i) scaled_sincos_uniform(x[i], 1.0, g_sc, s[i], c[i]);
+    for (long i = 0; i < n; ++i) sincos_uniform(x[i], g_sc, s[i], c[i]);
 }
 void fm_normal_pair(const uint32_t* xa, const uint32_t* xb, double* z0, double* z1, long n)
 {

@@ -191,14 +191,17 @@ __device__ __forceinline__ void collide(real (&g)[3][3][3], const StepParams<rea
             philox_call(ps, P.rng, call, w);
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
-                real z0, z1;
-                normal_pair(w[2 * h], w[2 * h + 1], lg, sc, z0, z1);
-                const int k = 4 + 4 * call + 2 * h;            // modes k (first) and k+1 (second), R8
+                real R, sn, cs;
+                normal_polar(w[2 * h], w[2 * h + 1], lg, sc, R, sn, cs);
+                const int k = 4 + 4 * call + 2 * h;            // modes k (first normal R cs) and k+1 (second, R sn), R8
+                const int ca = amp_class(mode_p(k), mode_q(k), mode_r(k));
                 real& m0 = Ms[mode_p(k)][mode_q(k)][mode_r(k)];
-                m0 = fma(amp[amp_class(mode_p(k), mode_q(k), mode_r(k))], z0, m0);
+                const real A0 = amp[ca] * R;                   // the FDT amplitude rides on the radius
+                m0 = fma(A0, cs, m0);
                 if (k + 1 < Q) {
+                    const int cb = amp_class(mode_p(k + 1), mode_q(k + 1), mode_r(k + 1));
                     real& m1 = Ms[mode_p(k + 1)][mode_q(k + 1)][mode_r(k + 1)];
-                    m1 = fma(amp[amp_class(mode_p(k + 1), mode_q(k + 1), mode_r(k + 1))], z1, m1);
+                    m1 = fma((cb == ca) ? A0 : amp[cb] * R, sn, m1);
                 }
             }
         }

@@ -119,12 +119,13 @@ __device__ __forceinline__ void philox_call(const PhiloxSite& P, const PhiloxSte
     out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
-// Box-Muller on two words.  fp64: 32-bit uniforms (x+0.5)/2^32 (exact in double, never 0 or 1); evaluated by the
-// table-driven branch-free routines of rflbm_fastmath.cuh (lg/sc: the tables, staged in shared memory).
-__device__ __forceinline__ void normal_pair(uint32_t xa, uint32_t xb, const f64x2* lg, const f64x2* sc, double& z0,
-                                            double& z1)
+// Box-Muller on two words, polar form: the normals are R*cs (first) and R*sn (second).  fp64: 32-bit uniforms
+// (x+0.5)/2^32 (exact in double, never 0 or 1); evaluated by the table-driven branch-free routines of
+// rflbm_fastmath.cuh (lg/sc: the tables, staged in shared memory).
+__device__ __forceinline__ void normal_polar(uint32_t xa, uint32_t xb, const f64x2* lg, const f64x2* sc, double& R,
+                                             double& sn, double& cs)
 {
-    normal_pair_fast(xa, xb, lg, sc, z0, z1);
+    normal_polar_fast(xa, xb, lg, sc, R, sn, cs);
 }
 
 // fp32 mode (R14): 24-bit uniforms ((x>>8)+0.5)/2^24, float arithmetic on the special-function unit.
@@ -135,7 +136,8 @@ __device__ __forceinline__ void normal_pair(uint32_t xa, uint32_t xb, const f64x
 //   (for u within 2^-10 of 1 the series 2v + v^2 of -2 ln(1-v), v = 1-u exact, replaces it: R error < 1e-5 everywhere)
 //   R = W rsqrt.approx(W)                (MUFU.RSQ, 2 ulp; W >= 5.9e-8 > 0)
 //   sin, cos(2 pi u) = -sin, -cos(2 pi u - pi), argument in (-pi, pi) where MUFU.SIN/COS are good to 2^-21.4
-__device__ __forceinline__ void normal_pair(uint32_t xa, uint32_t xb, const f64x2*, const f64x2*, float& z0, float& z1)
+__device__ __forceinline__ void normal_polar(uint32_t xa, uint32_t xb, const f64x2*, const f64x2*, float& R, float& sn,
+                                             float& cs)
 {
     const uint32_t k = xa >> 8;
     const float ua = ((float)k + 0.5f) * (1.0f / 16777216.0f);     // rounds to 1.0f for the last k: handled below
@@ -147,13 +149,22 @@ __device__ __forceinline__ void normal_pair(uint32_t xa, uint32_t xb, const f64x
         W = fmaf(v, v, 2.0f * v);                                   // so -2 ln(1-v) = 2v + v^2 + O(v^3 < 1e-9), v exact
     }
     asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(rs) : "f"(W));
-    const float R = W * rs;
+    R = W * rs;
     // 2 pi u - pi = 2 pi ((xb>>8) - 2^23 + 0.5) / 2^24, exact integer part
     const float th = ((float)((int)(xb >> 8) - 8388608) + 0.5f) * (6.283185307179586f / 16777216.0f);
     float s, c;
     __sincosf(th, &s, &c);
-    z0 = -R * c;
-    z1 = -R * s;
+    sn = -s;
+    cs = -c;
+}
+
+template <typename real>
+__device__ __forceinline__ void normal_pair(uint32_t xa, uint32_t xb, const f64x2* lg, const f64x2* sc, real& z0, real& z1)
+{
+    real R, sn, cs;
+    normal_polar(xa, xb, lg, sc, R, sn, cs);
+    z0 = R * cs;
+    z1 = R * sn;
 }
 
 }  // namespace rflbm_dev
