@@ -22,6 +22,7 @@ _lib = None
 
 Q = 27
 F64, F32 = 0, 1
+MODEL_REG, MODEL_BGK = 0, 1
 
 
 def build(force: bool = False) -> str:
@@ -69,6 +70,8 @@ def load():
     lib.rflbm_ref_equilibrium.argtypes = [dbl, pd, pd]
     lib.rflbm_ref_equilibrium.restype = None
     lib.rflbm_ref_collide_site.argtypes = [pd, dbl, dbl, u64, i32, pd, C.c_uint32, u64, pd]
+    lib.rflbm_ref_collide_site_bgk.argtypes = [pd, dbl, dbl, u64, i32, C.c_uint32, u64, pd]
+    lib.rflbm_ref_set_model.argtypes = [vp, i32]
     lib.rflbm_ref_moments_of.argtypes = [pd, pd]
     lib.rflbm_ref_moments_of.restype = None
     _lib = lib
@@ -117,6 +120,14 @@ def collide_site(g, tau, kT=0.0, seed=0, precision=F64, gacc=(0.0, 0.0, 0.0), si
     return out
 
 
+def collide_site_bgk(g, tau, kT=0.0, seed=0, precision=F64, site=0, t=0):
+    """BGK-FLBM (Eq.11) collision of one site."""
+    out = np.zeros(Q)
+    load().rflbm_ref_collide_site_bgk(np.ascontiguousarray(g, np.float64), float(tau), float(kT), int(seed),
+                                      precision, int(site), int(t), out)
+    return out
+
+
 def moments_of(f):
     out = np.zeros(Q)
     load().rflbm_ref_moments_of(np.ascontiguousarray(f, np.float64), out)
@@ -156,6 +167,9 @@ class Ref:
 
     def set_walls_z(self, on=True):
         self._ck(self.lib.rflbm_ref_set_walls_z(self.h, int(on)), "set_walls_z")
+
+    def set_model(self, model):
+        self._ck(self.lib.rflbm_ref_set_model(self.h, int(model)), "set_model")
 
     def set_force(self, gx, gy, gz):
         self._ck(self.lib.rflbm_ref_set_force(self.h, gx, gy, gz), "set_force")

@@ -18,6 +18,7 @@
  *   noise phi_k r_k, k=4..26     :93-99   Eq.8-9 (k=1..3 carry no noise, :95; R3)
  *   back-transform               :105     Eq.10 (== Eq.25+26, :225-229)
  *   final update                 :221     Eq.24  with omega_g = 1 (:215)
+ *   BGK-FLBM (comparison model)  :109-111 Eq.11 with Eq.6 (:85), in population space (f^eq: DESIGN.md R19)
  *   streaming                    :87      Eq.7   (periodic; bounce-back walls: DESIGN.md R12)
  *   body force (Guo, moment form): not in the paper, R13
  *   random numbers               : "standard normal" :95; generator + mapping: DESIGN.md R8
@@ -47,6 +48,9 @@
 
 #define REF_F64 0
 #define REF_F32 1
+
+#define REF_MODEL_REG 0   /* Reg-FLBM, Eq.24: the hot path                         */
+#define REF_MODEL_BGK 1   /* BGK-FLBM, Eq.11: the paper's comparison model      */
 
 /* ------------------------------------------------------------------ tables */
 
@@ -213,6 +217,7 @@ typedef struct rflbm_ref {
     uint64_t seed;
     int precision;
     int walls_z;
+    int model;    /* REF_MODEL_REG (Eq.24) or REF_MODEL_BGK (Eq.11) */
     double g[3];
     uint64_t t;
     int inited;
@@ -285,7 +290,16 @@ int rflbm_ref_set_walls_z(rflbm_ref_t *h, int on)
 int rflbm_ref_set_force(rflbm_ref_t *h, double gx, double gy, double gz)
 {
     if (!h || !isfinite(gx) || !isfinite(gy) || !isfinite(gz)) return REF_EINVAL;
+    if (h->model == REF_MODEL_BGK && (gx != 0.0 || gy != 0.0 || gz != 0.0)) return REF_EINVAL;
     h->g[0] = gx; h->g[1] = gy; h->g[2] = gz;
+    return REF_OK;
+}
+
+int rflbm_ref_set_model(rflbm_ref_t *h, int model)
+{
+    if (!h || (model != REF_MODEL_REG && model != REF_MODEL_BGK)) return REF_EINVAL;
+    if (model == REF_MODEL_BGK && (h->g[0] != 0.0 || h->g[1] != 0.0 || h->g[2] != 0.0)) return REF_EINVAL;
+    h->model = model;
     return REF_OK;
 }
 
@@ -402,6 +416,51 @@ static void collide(const rflbm_ref_t *h, const double g[Q], uint32_t site, uint
     }
 }
 
+/* BGK-FLBM, Eq.11, written in POPULATION space exactly as printed:
+ *     f*_i = f_i^eq + (1 - omega) f_i^neq + w_i sum_k e_ki phi_k r_k / b_k,   f^neq = f - f^eq   (Eq.6 :85)
+ * with ONE relaxation rate omega = 1/tau for every non-conserved mode, hence phi_k of Eq.9 (:99) at that omega
+ * for all k = 4..26 (:95).  f^eq is not printed in Sec. II.A; reading R19: the same Hermite
+ * equilibrium f^(0) of Eq.25 with Eq.20 that Reg-FLBM uses, so that the two models differ only in what happens
+ * to the non-equilibrium part.  No body force in this model (the paper has none). */
+static void collide_bgk(const rflbm_ref_t *h, const double g[Q], uint32_t site, uint64_t t, double fstar[Q])
+{
+    const double omega = 1.0 / h->tau;
+    const double cs2 = 1.0 / 3.0;
+    double rho = 0.0, u[3] = {0.0, 0.0, 0.0};
+    for (int i = 0; i < Q; i++) rho += g[i];
+    for (int a = 0; a < 3; a++) {
+        for (int i = 0; i < Q; i++) u[a] += g[i] * (double)T_c[i][a];
+        u[a] = u[a] / rho;
+    }
+    double feq[Q];
+    rflbm_ref_equilibrium(rho, u, feq);
+    for (int i = 0; i < Q; i++) fstar[i] = feq[i] + (1.0 - omega) * (g[i] - feq[i]);
+    if (h->kT > 0.0) {
+        uint32_t words[24];
+        double r[Q], noise[Q];
+        draw_site(h->seed, t, site, h->precision, words, r);
+        for (int k = 0; k < Q; k++) noise[k] = 0.0;
+        for (int k = 4; k < Q; k++) noise[k] = sqrt(rho * h->kT * omega * (2.0 - omega) * T_b[k] / cs2) * r[k];
+        for (int i = 0; i < Q; i++) {
+            double s = 0.0;
+            for (int k = 4; k < Q; k++) s += noise[k] * T_e[k][i] / T_b[k];
+            fstar[i] += T_w[i] * s;
+        }
+    }
+}
+
+/* single-site entry for the pin tests: BGK-FLBM */
+int rflbm_ref_collide_site_bgk(const double g[Q], double tau, double kT, uint64_t seed, int precision,
+                               uint32_t site, uint64_t t, double fstar[Q])
+{
+    build_tables();
+    rflbm_ref_t h;
+    memset(&h, 0, sizeof(h));
+    h.tau = tau; h.kT = kT; h.seed = seed; h.precision = precision; h.model = REF_MODEL_BGK;
+    collide_bgk(&h, g, site, t, fstar);
+    return REF_OK;
+}
+
 /* single-site entry for the pin tests: collide with explicit parameters */
 int rflbm_ref_collide_site(const double g[Q], double tau, double kT, uint64_t seed, int precision,
                            const double gacc[3], uint32_t site, uint64_t t, double fstar[Q])
@@ -458,7 +517,8 @@ static void step_once(rflbm_ref_t *h, int reverse_order)
                 size_t s = (size_t)x + (size_t)nx * ((size_t)y + (size_t)ny * z);
                 double g[Q], fs[Q];
                 for (int i = 0; i < Q; i++) g[i] = S[(size_t)i * n + s];      /* 1. */
-                collide(h, g, (uint32_t)s, h->t, fs);                          /* 2.-7. */
+                if (h->model == REF_MODEL_BGK) collide_bgk(h, g, (uint32_t)s, h->t, fs);
+                else collide(h, g, (uint32_t)s, h->t, fs);                     /* 2.-7. */
                 for (int i = 0; i < Q; i++) {                                  /* 8. stream, Eq.7 */
                     int xd = wrap(x + T_c[i][0], nx);
                     int yd = wrap(y + T_c[i][1], ny);
