@@ -72,6 +72,15 @@ int rflbm_init(rflbm_t* h, const void* rho_dev, const void* u_dev);
  * rflbm_step(a); rflbm_step(b) is bit-identical to rflbm_step(a+b).  ESTATE before init. */
 int rflbm_step(rflbm_t* h, int nsteps);
 
+/* Collision model.  RFLBM_MODEL_REG (default): the regularized fluctuating model, Eq.24, the hot
+ * path.  RFLBM_MODEL_BGK: the paper's comparison model BGK-FLBM, Eq.11 (:109-111) with Eq.6 (:85): every
+ * non-conserved mode k = 4..26 relaxes at the one rate omega = 1/tau and carries noise of amplitude Eq.9 at that
+ * omega; f^eq is the Hermite equilibrium of Eq.25 (reading R19).  May be changed between steps (the state is the
+ * populations).  EINVAL: unknown model, or BGK with a body force set (and rflbm_set_force refuses a non-zero
+ * force while the model is BGK). */
+enum { RFLBM_MODEL_REG = 0, RFLBM_MODEL_BGK = 1 };
+int rflbm_set_model(rflbm_t* h, int model);
+
 /* Which implementation of the step kernel rflbm_step launches.  AUTO (default): the TMA-staged kernel when the
  * lattice allows it (nx >= 128 and nx*sizeof(real) a multiple of 16), else the plain one-thread-per-site kernel.  PLAIN forces the
  * latter; TMA fails with EINVAL at rflbm_step if the lattice does not allow it.  All variants compute the same

@@ -12,6 +12,7 @@ import os
 F64, F32 = 0, 1
 OK, EINVAL, ESTATE, ENOMEM, ECUDA = 0, -1, -2, -3, -4
 KERNEL_AUTO, KERNEL_PLAIN, KERNEL_TMA = 0, 1, 2
+MODEL_REG, MODEL_BGK = 0, 1
 Q = 27
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -28,6 +29,7 @@ SYMBOLS = {
     "rflbm_set_walls_z": (_i32, [_vp, _i32]),
     "rflbm_set_force": (_i32, [_vp, _dbl, _dbl, _dbl]),
     "rflbm_set_kernel_variant": (_i32, [_vp, _i32]),
+    "rflbm_set_model": (_i32, [_vp, _i32]),
     "rflbm_init": (_i32, [_vp, _vp, _vp]),
     "rflbm_step": (_i32, [_vp, _i32]),
     "rflbm_moments": (_i32, [_vp, _vp, _vp]),
@@ -117,6 +119,9 @@ class Rflbm:
 
     def set_walls_z(self, on=True):
         self._ck(self.lib.rflbm_set_walls_z(self.h, int(on)))
+
+    def set_model(self, model):
+        self._ck(self.lib.rflbm_set_model(self.h, int(model)))
 
     def set_kernel_variant(self, variant):
         self._ck(self.lib.rflbm_set_kernel_variant(self.h, int(variant)))

@@ -25,6 +25,7 @@ struct rflbm {
     uint64_t seed;
     int precision;
     int walls;
+    int model;           // RFLBM_MODEL_REG / RFLBM_MODEL_BGK
     double g[3];
     bool force;
     void* ws;            // borrowed workspace
@@ -197,6 +198,8 @@ extern "C" int rflbm_set_force(rflbm_t* h, double gx, double gy, double gz)
 {
     if (!h) return RFLBM_EINVAL;
     if (!std::isfinite(gx) || !std::isfinite(gy) || !std::isfinite(gz)) return fail(h, RFLBM_EINVAL, "non-finite force");
+    if (h->model == RFLBM_MODEL_BGK && (gx != 0.0 || gy != 0.0 || gz != 0.0))
+        return fail(h, RFLBM_EINVAL, "BGK-FLBM carries no body force");
     h->g[0] = gx; h->g[1] = gy; h->g[2] = gz;
     h->force = (gx != 0.0 || gy != 0.0 || gz != 0.0);
     return RFLBM_OK;
@@ -220,7 +223,9 @@ static StepParams<real> step_params(const rflbm* h, uint64_t t)
     P.nx = h->nx; P.ny = h->ny; P.nz = h->nz; P.N = h->N; P.QS = h->QS;
     P.half_omc = (real)(0.5 * (1.0 - omega));
     // Eq.9 per unit sqrt(rho): sqrt(3 kT omega_k (2 - omega_k)) prod_axis s_p, s = (1, sqrt3/6, sqrt2/6)
-    const double nh = std::sqrt(3.0 * h->kT * omega * (2.0 - omega)), ng = std::sqrt(3.0 * h->kT);
+    // omega_k = omega_h for k = 4..9; ghosts: 1 in Reg-FLBM (:215), the same omega in BGK-FLBM (Eq.11)
+    const double nh = std::sqrt(3.0 * h->kT * omega * (2.0 - omega));
+    const double ng = (h->model == RFLBM_MODEL_BGK) ? nh : std::sqrt(3.0 * h->kT);
     const double s1 = std::sqrt(3.0) / 6.0, s2 = std::sqrt(2.0) / 6.0;
     P.amp[AMP_200] = (real)(nh * s2);
     P.amp[AMP_110] = (real)(nh * s1 * s1);
@@ -308,66 +313,53 @@ extern "C" int rflbm_get_populations(rflbm_t* h, void* f_dev)
 }
 
 // ---------------------------------------------------------------- the time step
-template <typename real, bool WALLS, bool FORCE, bool NOISE>
-static void launch_step(rflbm* h, const StepParams<real>& P)
+template <typename real, bool WALLS, bool FORCE, bool NOISE, bool BGK>
+static void launch_one(rflbm* h, const StepParams<real>& P, bool tma)
 {
-    step_kernel<real, WALLS, FORCE, NOISE>
-        <<<h->grid, h->block, 0, h->stream>>>((const real*)h->buf[h->cur], (real*)h->buf[h->cur ^ 1], P);
-}
-
-template <typename real, bool WALLS, bool FORCE, bool NOISE>
-static void launch_step_tma(rflbm* h, const StepParams<real>& P)
-{
-    const dim3 grid((h->nx + TILE_X - 1) / TILE_X, (h->ny + h->tma_rows - 1) / h->tma_rows, h->nz);
-    step_kernel_tma<real, WALLS, FORCE, NOISE><<<grid, TILE_X, 0, h->stream>>>(
-        h->tmap[h->cur], (const real*)h->buf[h->cur], (real*)h->buf[h->cur ^ 1], P, h->tma_rows);
+    if (tma) {
+        const dim3 grid((h->nx + TILE_X - 1) / TILE_X, (h->ny + h->tma_rows - 1) / h->tma_rows, h->nz);
+        step_kernel_tma<real, WALLS, FORCE, NOISE, BGK><<<grid, TILE_X, 0, h->stream>>>(
+            h->tmap[h->cur], (const real*)h->buf[h->cur], (real*)h->buf[h->cur ^ 1], P, h->tma_rows);
+    } else {
+        step_kernel<real, WALLS, FORCE, NOISE, BGK>
+            <<<h->grid, h->block, 0, h->stream>>>((const real*)h->buf[h->cur], (real*)h->buf[h->cur ^ 1], P);
+    }
 }
 
 static bool use_tma(const rflbm* h) { return h->tma_ok && h->variant != RFLBM_KERNEL_PLAIN; }
 
+// variant bits: 8 = BGK-FLBM, 4 = walls, 2 = force, 1 = noise (BGK carries no force: rflbm_set_model / set_force)
 template <typename real>
-static void dispatch_tma(rflbm* h, const StepParams<real>& P, int variant)
+static void dispatch_step(rflbm* h, const StepParams<real>& P, int variant, bool tma)
 {
     switch (variant) {
-        case 0: launch_step_tma<real, false, false, false>(h, P); break;
-        case 1: launch_step_tma<real, false, false, true>(h, P); break;
-        case 2: launch_step_tma<real, false, true, false>(h, P); break;
-        case 3: launch_step_tma<real, false, true, true>(h, P); break;
-        case 4: launch_step_tma<real, true, false, false>(h, P); break;
-        case 5: launch_step_tma<real, true, false, true>(h, P); break;
-        case 6: launch_step_tma<real, true, true, false>(h, P); break;
-        default: launch_step_tma<real, true, true, true>(h, P); break;
+        case 0: launch_one<real, false, false, false, false>(h, P, tma); break;
+        case 1: launch_one<real, false, false, true, false>(h, P, tma); break;
+        case 2: launch_one<real, false, true, false, false>(h, P, tma); break;
+        case 3: launch_one<real, false, true, true, false>(h, P, tma); break;
+        case 4: launch_one<real, true, false, false, false>(h, P, tma); break;
+        case 5: launch_one<real, true, false, true, false>(h, P, tma); break;
+        case 6: launch_one<real, true, true, false, false>(h, P, tma); break;
+        case 7: launch_one<real, true, true, true, false>(h, P, tma); break;
+        case 8: launch_one<real, false, false, false, true>(h, P, tma); break;
+        case 9: launch_one<real, false, false, true, true>(h, P, tma); break;
+        case 12: launch_one<real, true, false, false, true>(h, P, tma); break;
+        default: launch_one<real, true, false, true, true>(h, P, tma); break;     // 13
     }
 }
 
 template <typename real>
 static int do_step(rflbm* h, int nsteps)
 {
-    const bool noise = h->kT > 0.0;       // kT = 0: deterministic Reg-LBM, RNG skipped entirely (R17)
+    const bool noise = h->kT > 0.0;       // kT = 0: deterministic (Reg-)LBM, RNG skipped entirely (R17)
     if (h->variant == RFLBM_KERNEL_TMA && !h->tma_ok)
         return fail(h, RFLBM_EINVAL, "TMA kernel needs nx >= 128 and a row pitch that is a multiple of 16 bytes");
+    const bool tma = use_tma(h);
+    const int variant = (h->model == RFLBM_MODEL_BGK ? 8 : 0) | (h->walls ? 4 : 0) | (h->force ? 2 : 0) | (noise ? 1 : 0);
     for (int s = 0; s < nsteps; ++s) {
         const StepParams<real> P = step_params<real>(h, h->t);
-        const int variant = (h->walls ? 4 : 0) | (h->force ? 2 : 0) | (noise ? 1 : 0);
-        if (use_tma(h)) {
-            dispatch_tma<real>(h, P, variant);
-            const int rc = after_launch(h, "step_kernel_tma");
-            if (rc != RFLBM_OK) return rc;
-            h->cur ^= 1;
-            h->t += 1;
-            continue;
-        }
-        switch (variant) {
-            case 0: launch_step<real, false, false, false>(h, P); break;
-            case 1: launch_step<real, false, false, true>(h, P); break;
-            case 2: launch_step<real, false, true, false>(h, P); break;
-            case 3: launch_step<real, false, true, true>(h, P); break;
-            case 4: launch_step<real, true, false, false>(h, P); break;
-            case 5: launch_step<real, true, false, true>(h, P); break;
-            case 6: launch_step<real, true, true, false>(h, P); break;
-            default: launch_step<real, true, true, true>(h, P); break;
-        }
-        const int rc = after_launch(h, "step_kernel");
+        dispatch_step<real>(h, P, variant, tma);
+        const int rc = after_launch(h, tma ? "step_kernel_tma" : "step_kernel");
         if (rc != RFLBM_OK) return rc;
         h->cur ^= 1;
         h->t += 1;
@@ -499,6 +491,15 @@ extern "C" int rflbm_run_host(rflbm_t* h, const void* rho_host, const void* u_ho
     rc = check_cuda(h, cudaMemcpyAsync(u_out_host, d_u, 3 * fb, cudaMemcpyDeviceToHost, h->stream), "D2H u");
     if (rc != RFLBM_OK) return rc;
     return check_cuda(h, cudaStreamSynchronize(h->stream), "cudaStreamSynchronize");
+}
+
+extern "C" int rflbm_set_model(rflbm_t* h, int model)
+{
+    if (!h) return RFLBM_EINVAL;
+    if (model != RFLBM_MODEL_REG && model != RFLBM_MODEL_BGK) return fail(h, RFLBM_EINVAL, "unknown model %d", model);
+    if (model == RFLBM_MODEL_BGK && h->force) return fail(h, RFLBM_EINVAL, "BGK-FLBM carries no body force");
+    h->model = model;
+    return RFLBM_OK;
 }
 
 extern "C" int rflbm_set_kernel_variant(rflbm_t* h, int variant)

@@ -106,6 +106,36 @@ __device__ __forceinline__ Moments10<real> forward_moments(const real (&g)[3][3]
     return m;
 }
 
+// full forward transform (Eq.4, separable): m[p][q][r] = sum_i H_p(cx) H_q(cy) H_r(cz) g_i, raw (unscaled) moments.
+// 1-D: m0 = f- + f0 + f+, m1 = f+ - f-, m2 = (f+ + f-) - m0/3.  Needed by BGK-FLBM only (Eq.11).
+template <typename real>
+__device__ __forceinline__ void fwd1d(real fm, real f0, real fp, real& m0, real& m1, real& m2)
+{
+    const real s = fp + fm;
+    m1 = fp - fm;
+    m0 = s + f0;
+    m2 = fma(real(-1.0 / 3.0), m0, s);
+}
+
+template <typename real>
+__device__ __forceinline__ void forward_all(const real (&g)[3][3][3], real (&m)[3][3][3])
+{
+    real X[3][3][3];   // [cz][cy][p]
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int b = 0; b < 3; ++b) fwd1d(g[c][b][0], g[c][b][1], g[c][b][2], X[c][b][0], X[c][b][1], X[c][b][2]);
+    real Y[3][3][3];   // [cz][q][p]
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int p = 0; p < 3; ++p) fwd1d(X[c][0][p], X[c][1][p], X[c][2][p], Y[c][0][p], Y[c][1][p], Y[c][2][p]);
+#pragma unroll
+    for (int q = 0; q < 3; ++q)
+#pragma unroll
+        for (int p = 0; p < 3; ++p) fwd1d(Y[0][q][p], Y[1][q][p], Y[2][q][p], m[p][q][0], m[p][q][1], m[p][q][2]);
+}
+
 // 1-D back-transform of (m0, m1/2, m2/2) -> values at c = -1, 0, +1 (see the header comment)
 template <typename real>
 __device__ __forceinline__ void back1d(real m0, real m1s, real m2s, real& fm, real& f0, real& fp)
@@ -117,11 +147,23 @@ __device__ __forceinline__ void back1d(real m0, real m1s, real m2s, real& fm, re
 }
 
 // In: g = pre-collision populations of the site.  Out: g = post-collision populations f*.
-template <typename real, bool FORCE, bool NOISE>
+// BGK = false: Reg-FLBM, Eq.24 (the hot path).  BGK = true: BGK-FLBM, Eq.11 (:109-111), the paper's comparison
+// model: every non-conserved mode relaxes at the one rate omega, M_k = M_k^eq + (1-omega)(m_k - M_k^eq), which
+// needs all 27 moments of the incoming populations (no body force in this model).
+template <typename real, bool FORCE, bool NOISE, bool BGK = false>
 __device__ __forceinline__ void collide(real (&g)[3][3][3], const StepParams<real>& P, uint32_t site,
                                         const f64x2* lg, const f64x2* sc)
 {
-    const Moments10<real> m = forward_moments(g);
+    static_assert(!(BGK && FORCE), "BGK-FLBM carries no body force");
+    Moments10<real> m;
+    real mall[3][3][3];
+    if (BGK) {
+        forward_all(g, mall);
+        m.rho = mall[0][0][0]; m.jx = mall[1][0][0]; m.jy = mall[0][1][0]; m.jz = mall[0][0][1];
+        m.pxx = m.pyy = m.pzz = m.pxy = m.pxz = m.pyz = real(0);     // unused in this branch
+    } else {
+        m = forward_moments(g);
+    }
 
     // Eq.3 (with the half-force shift of R13)
     const real inv_rho = rcp_pos<real>(m.rho);
@@ -147,6 +189,22 @@ __device__ __forceinline__ void collide(real (&g)[3][3][3], const StepParams<rea
         }
     }
 
+    if (BGK) {
+        // Ms_k = E_k + (1-omega)(2^-nnz m_k - E_k) = (1-omega) 2^-nnz m_k + omega E_k for k = 4..26
+        const real om = real(1.0) - real(2.0) * P.half_omc;
+        const real w2 = P.half_omc, w4 = real(0.5) * P.half_omc, w8 = real(0.25) * P.half_omc;
+#pragma unroll
+        for (int p = 0; p < 3; ++p)
+#pragma unroll
+            for (int q = 0; q < 3; ++q)
+#pragma unroll
+                for (int r = 0; r < 3; ++r) {
+                    const int nnz = (p > 0) + (q > 0) + (r > 0);
+                    if (p + q + r < 2) continue;                     // conserved modes keep their equilibrium value
+                    const real w = (nnz == 1) ? w2 : (nnz == 2) ? w4 : w8;
+                    Ms[p][q][r] = fma(w, mall[p][q][r], om * Ms[p][q][r]);
+                }
+    } else
     // stress modes k = 4..9: Eq.19 a_1,ab = sum_i g_i (c_a c_b - delta_ab/3) - rho u_a u_b, relaxed by (1-omega_h)
     // (Eq.26).  Scaled: diagonal E + (1-omega_h)/2 (p_aa - rho/3 - 2E), E = rho u_a^2/2;
     //           off-diagonal E + (1-omega_h)/4 (p_ab - 4E), E = rho u_a u_b/4.

@@ -68,7 +68,7 @@ __device__ __forceinline__ void stage_tables(const f64x2* __restrict__ tab, f64x
 }
 
 // ---------------------------------------------------------------- the hot kernel: one time step
-template <typename real, bool WALLS, bool FORCE, bool NOISE>
+template <typename real, bool WALLS, bool FORCE, bool NOISE, bool BGK>
 __global__ void __launch_bounds__(128)
 step_kernel(const real* __restrict__ src, real* __restrict__ dst, const __grid_constant__ StepParams<real> P)
 {
@@ -80,7 +80,7 @@ step_kernel(const real* __restrict__ src, real* __restrict__ dst, const __grid_c
     if (WALLS && (i.z == 0 || i.z == P.nz - 1)) return;    // solid layers are never updated
     real g[3][3][3];
     gather<real, WALLS>(src, P.QS, P.nx, P.ny, P.nz, i, g);
-    collide<real, FORCE, NOISE>(g, P, (uint32_t)i.s, s_tab, s_tab + LOG_TABLE_N);
+    collide<real, FORCE, NOISE, BGK>(g, P, (uint32_t)i.s, s_tab, s_tab + LOG_TABLE_N);
 #pragma unroll
     for (int c = 0; c < 3; ++c)
 #pragma unroll

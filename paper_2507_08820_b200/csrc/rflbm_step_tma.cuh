@@ -109,7 +109,7 @@ __device__ __forceinline__ void issue_tile(const CUtensorMap* tmap, uint32_t s_i
 }
 
 // fp64: 128 registers, 41 KB -> 4 blocks per SM; fp32: 64 registers, 15 KB -> 8 blocks per SM
-template <typename real, bool WALLS, bool FORCE, bool NOISE>
+template <typename real, bool WALLS, bool FORCE, bool NOISE, bool BGK>
 __global__ void __launch_bounds__(TILE_X, sizeof(real) == 8 ? 4 : 8)
 step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const real* __restrict__ src, real* __restrict__ dst,
                 const __grid_constant__ StepParams<real> P, int rows)
@@ -205,7 +205,7 @@ step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const real* __rest
             }
         }
         if (active) {
-            collide<real, FORCE, NOISE>(g, P, (uint32_t)s, s_tab, s_tab + LOG_TABLE_N);
+            collide<real, FORCE, NOISE, BGK>(g, P, (uint32_t)s, s_tab, s_tab + LOG_TABLE_N);
             const unsigned long long out = reinterpret_cast<unsigned long long>(dst + s);
 #pragma unroll
             for (int c = 0; c < 3; ++c)

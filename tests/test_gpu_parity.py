@@ -245,3 +245,44 @@ def test_tma_variant_rejected_when_lattice_does_not_allow_it():
     with pytest.raises(binding.RflbmError) as e:
         sim.step(1)
     assert e.value.code == binding.EINVAL
+
+
+@pytest.mark.parametrize("shape,prec,walls,kT,tau", [((16, 16, 16), binding.F64, False, 1e-4, 1.0), ((5, 7, 9), binding.F64, False, 1e-4, 0.55),
+                                                    ((132, 6, 5), binding.F64, True, 1e-4, 0.8), ((256, 4, 3), binding.F64, False, 0.0, 3.0),
+                                                    ((20, 12, 7), binding.F32, False, 1e-4, 0.7), ((136, 5, 6), binding.F32, True, 1e-4, 0.9)])
+def test_bgk_flbm_model_matches_oracle(shape, prec, walls, kT, tau):
+    """BGK-FLBM (Eq.11), the paper's comparison model: GPU mode-space form against the oracle's population-space
+    form, 100 steps, plain and (where the lattice allows) TMA kernel bit-identical."""
+    torch = torch_()
+    nx, ny, nz = shape
+    fields = synthetic.smooth_random_fields(nx, ny, nz, 23)
+    outs = []
+    variants = [binding.KERNEL_PLAIN] + ([binding.KERNEL_TMA] if nx >= 128 else [])
+    for variant in variants:
+        sim, ref = make_pair(nx, ny, nz, tau, kT, 29, precision=prec, walls=walls)
+        sim.set_model(binding.MODEL_BGK); ref.set_model(oracle.MODEL_BGK)
+        sim.set_kernel_variant(variant)
+        init_pair(sim, ref, fields)
+        sim.step(100)
+        outs.append(sim.get_populations())
+    ref.step(100)
+    if len(outs) == 2:
+        assert torch.equal(outs[0], outs[1])
+    err = np.abs(outs[0].cpu().numpy().astype(np.float64) - ref.get_populations()).max()
+    assert err < (TOL64 if prec == binding.F64 else TOL32), err
+    d = sim.diagnostics()
+    assert abs(d[0] - ref.diagnostics()[0]) < (1e-9 if prec == binding.F64 else 1e-2)
+
+
+def test_bgk_model_refuses_force_and_differs_from_reg():
+    sim = binding.Rflbm(8, 8, 8, 0.8, 1e-4, 1.0, 3)
+    sim.set_model(binding.MODEL_BGK)
+    with pytest.raises(binding.RflbmError) as e:
+        sim.set_force(1e-6, 0.0, 0.0)
+    assert e.value.code == binding.EINVAL
+    with pytest.raises(binding.RflbmError):
+        sim.set_model(5)
+    sim.init(); sim.step(20)
+    reg = binding.Rflbm(8, 8, 8, 0.8, 1e-4, 1.0, 3)
+    reg.init(); reg.step(20)
+    assert (sim.get_populations() - reg.get_populations()).abs().max().item() > 1e-6
