@@ -175,3 +175,35 @@ def test_config5_channel_fp32_startup_profile_256():
     print("near-wall <du^2>/kT (layers 1..3):", v[:, :3])
     d1 = sim.diagnostics()
     assert abs(d1[0] / d0[0] - 1.0) < 1e-5                           # fp32 storage: mass drift reported and bounded
+
+
+@pytest.mark.parametrize("model,tau", [("reg", 0.51), ("reg", 1.0), ("reg", 50.0), ("bgk", 1.0), ("bgk", 50.0)])
+def test_table_III_trend_equilibration_ratios_64(model, tau):
+    """Reduced-scale Table III (64^3 and 2e4 steps instead of 256^3 and 5e5, kT = 1/3000 as in
+    :254): ER of rho, momentum, diagonal and off-diagonal Hermite stress = variance / (rho0 kT b_k / cs2).
+    Reg-FLBM: within 0.5 % of 1 for 0.51 <= tau <= 100 (:260), reproduced here.
+    BGK-FLBM with reading R19 (all 23 modes thermalised at the one omega) ALSO equilibrates to 1.000 at tau = 50;
+    the paper's BGK column (0.953 / 0.930 at tau >= 50) is not reproduced by Eq.11 as printed — DESIGN.md section 10."""
+    torch = torch_()
+    n, kT = 64, 1.0 / 3000.0
+    c = torch.tensor(oracle.tables()[0], dtype=torch.float64, device="cuda")
+    sim = binding.Rflbm(n, n, n, tau, kT, 1.0, 9)
+    sim.set_model(binding.MODEL_BGK if model == "bgk" else binding.MODEL_REG)
+    sim.init()
+    sim.step(4000)
+    er = []
+    while sim.step_count <= 20000:
+        f = sim.get_populations().reshape(27, -1)
+        rho = f.sum(0)
+        j = c.T @ f
+        pd = torch.stack([((c[:, a] ** 2 - 1.0 / 3.0)[:, None] * f).sum(0) for a in range(3)])
+        po = torch.stack([((c[:, a] * c[:, b])[:, None] * f).sum(0) for a, b in ((0, 1), (0, 2), (1, 2))])
+        er.append([float(rho.var(unbiased=False)) / (3 * kT), float(j.var(dim=1, unbiased=False).mean()) / kT,
+                   float(pd.var(dim=1, unbiased=False).mean()) / (2.0 / 3.0 * kT),
+                   float(po.var(dim=1, unbiased=False).mean()) / (1.0 / 3.0 * kT)])
+        sim.step(200)
+    er = np.mean(er, axis=0)
+    print(model, tau, "ER(rho, j, Pi_aa, Pi_ab) =", np.round(er, 4))
+    # tau = 0.51 sits at the edge of the paper's 0.5 % band: Table III prints 1.005 / 1.013 / 1.004 / 1.012 there
+    # (measured here: 1.003 / 1.006 / 1.006 / 1.005)
+    assert np.abs(er - 1.0).max() < (0.015 if tau < 0.55 else 0.005), er
