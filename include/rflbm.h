@@ -91,6 +91,11 @@ int rflbm_set_kernel_variant(rflbm_t* h, int variant);
 /* rho[N], u[3][N] (device, `real`) of the current state: Eq.2-3, u = (j + F/2)/rho.  Solid nodes: 0. */
 int rflbm_moments(rflbm_t* h, void* rho_dev, void* u_dev);
 
+/* pi[6][N] (device, `real`): momentum-flux tensor Pi_ab = a_0,ab + a_1,ab = sum_i f_i (c_ia c_ib - delta_ab/3) of the
+ * current state (Eq.18-19; the quantity the paper snapshots, :252, :260), order xx, yy, zz, xy, xz,
+ * yz.  Solid nodes: 0. */
+int rflbm_stress(rflbm_t* h, void* pi_dev);
+
 /* Synchronises the stream.  out_host = { sum rho, sum rho u_x,y,z, mean u_x,y,z, var u_x,y,z } over fluid sites
  * (warp-shuffle + block reduction, fp64 accumulation). */
 int rflbm_diagnostics(rflbm_t* h, double out_host[10]);

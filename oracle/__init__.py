@@ -59,6 +59,7 @@ def load():
     lib.rflbm_ref_step_reversed.argtypes = [vp, i32]
     lib.rflbm_ref_moments.argtypes = [vp, pd, pd]
     lib.rflbm_ref_diagnostics.argtypes = [vp, pd]
+    lib.rflbm_ref_stress.argtypes = [vp, pd]
     lib.rflbm_ref_get_populations.argtypes = [vp, pd]
     lib.rflbm_ref_set_populations.argtypes = [vp, pd, u64]
     lib.rflbm_ref_debug_rng.argtypes = [vp, u64, pu32, pd]
@@ -197,6 +198,11 @@ class Ref:
         u = np.zeros((3,) + self.shape)
         self._ck(self.lib.rflbm_ref_moments(self.h, rho, u), "moments")
         return rho, u
+
+    def stress(self):
+        pi = np.zeros((6,) + self.shape)
+        self._ck(self.lib.rflbm_ref_stress(self.h, pi), "stress")
+        return pi
 
     def diagnostics(self):
         out = np.zeros(10)

@@ -583,6 +583,28 @@ int rflbm_ref_moments(rflbm_ref_t *h, double *rho, double *u)
     return REF_OK;
 }
 
+/* Momentum-flux tensor the paper saves with its snapshots and uses for Table III (:260):
+ * Pi_ab = a_0,ab^(2) + a_1,ab^(2) = sum_i f_i (c_ia c_ib - cs2 delta_ab)  (Eq.18 :150 + Eq.19 :153; the rho u u
+ * terms cancel).  pi[6][N] in the order xx, yy, zz, xy, xz, yz (modes k = 4..9 of Table II); solid nodes: 0. */
+int rflbm_ref_stress(rflbm_ref_t *h, double *pi)
+{
+    if (!h || !pi) return REF_EINVAL;
+    if (!h->inited) return REF_ESTATE;
+    static const int AB[6][2] = {{0, 0}, {1, 1}, {2, 2}, {0, 1}, {0, 2}, {1, 2}};
+    const size_t n = nsites(h);
+    for (int z = 0; z < h->nz; z++)
+        for (size_t s = (size_t)z * h->nx * h->ny; s < (size_t)(z + 1) * h->nx * h->ny; s++)
+            for (int m = 0; m < 6; m++) {
+                double v = 0.0;
+                if (!is_solid(h, z))
+                    for (int i = 0; i < Q; i++)
+                        v += h->S[(size_t)i * n + s] *
+                             ((double)(T_c[i][AB[m][0]] * T_c[i][AB[m][1]]) - (AB[m][0] == AB[m][1] ? 1.0 / 3.0 : 0.0));
+                pi[(size_t)m * n + s] = v;
+            }
+    return REF_OK;
+}
+
 /* out = { sum rho, sum rho u_x,y,z, mean u_x,y,z, var u_x,y,z } over fluid sites */
 int rflbm_ref_diagnostics(rflbm_ref_t *h, double out[10])
 {

@@ -33,6 +33,7 @@ SYMBOLS = {
     "rflbm_init": (_i32, [_vp, _vp, _vp]),
     "rflbm_step": (_i32, [_vp, _i32]),
     "rflbm_moments": (_i32, [_vp, _vp, _vp]),
+    "rflbm_stress": (_i32, [_vp, _vp]),
     "rflbm_diagnostics": (_i32, [_vp, C.POINTER(_dbl)]),
     "rflbm_get_populations": (_i32, [_vp, _vp]),
     "rflbm_set_populations": (_i32, [_vp, _vp, _u64]),
@@ -152,6 +153,12 @@ class Rflbm:
             u = t.empty((3,) + self.shape, dtype=self.dtype, device=self.device)
         self._ck(self.lib.rflbm_moments(self.h, rho.data_ptr(), u.data_ptr()))
         return rho, u
+
+    def stress(self, pi=None):
+        if pi is None:
+            pi = self.torch.empty((6,) + self.shape, dtype=self.dtype, device=self.device)
+        self._ck(self.lib.rflbm_stress(self.h, pi.data_ptr()))
+        return pi
 
     def diagnostics(self):
         out = (_dbl * 10)()

@@ -396,6 +396,25 @@ extern "C" int rflbm_moments(rflbm_t* h, void* rho_dev, void* u_dev)
 }
 
 template <typename real>
+static int do_stress(rflbm* h, void* pi)
+{
+    const FieldParams<real> P = field_params<real>(h);
+    if (h->walls)
+        stress_kernel<real, true><<<h->grid, h->block, 0, h->stream>>>((const real*)h->buf[h->cur], (real*)pi, P);
+    else
+        stress_kernel<real, false><<<h->grid, h->block, 0, h->stream>>>((const real*)h->buf[h->cur], (real*)pi, P);
+    return after_launch(h, "stress_kernel");
+}
+
+extern "C" int rflbm_stress(rflbm_t* h, void* pi_dev)
+{
+    if (!h) return RFLBM_EINVAL;
+    if (!pi_dev) return fail(h, RFLBM_EINVAL, "pi_dev is NULL");
+    if (!h->inited) return fail(h, RFLBM_ESTATE, "rflbm_stress before init");
+    return (h->precision == RFLBM_F64) ? do_stress<double>(h, pi_dev) : do_stress<float>(h, pi_dev);
+}
+
+template <typename real>
 static int do_diagnostics(rflbm* h)
 {
     const FieldParams<real> P = field_params<real>(h);

@@ -119,6 +119,27 @@ moments_kernel(const real* __restrict__ src, real* __restrict__ rho, real* __res
     u[2 * P.N + i.s] = fma(m.jz, inv, P.hgz);
 }
 
+// Pi_ab = sum_i f_i (c_a c_b - delta_ab/3) of the current state (Eq.18 + Eq.19):
+// pi[6][N] in the order xx, yy, zz, xy, xz, yz.  Solid nodes: 0.
+template <typename real, bool WALLS>
+__global__ void __launch_bounds__(128)
+stress_kernel(const real* __restrict__ src, real* __restrict__ pi, const FieldParams<real> P)
+{
+    const SiteIndex i = my_site(P.nx, P.ny);
+    if (!i.valid) return;
+    real v[6] = {real(0), real(0), real(0), real(0), real(0), real(0)};
+    if (!(WALLS && (i.z == 0 || i.z == P.nz - 1))) {
+        real g[3][3][3];
+        gather<real, WALLS>(src, P.QS, P.nx, P.ny, P.nz, i, g);
+        const Moments10<real> m = forward_moments(g);
+        const real third = m.rho * real(1.0 / 3.0);
+        v[0] = m.pxx - third; v[1] = m.pyy - third; v[2] = m.pzz - third;
+        v[3] = m.pxy; v[4] = m.pxz; v[5] = m.pyz;
+    }
+#pragma unroll
+    for (int n = 0; n < 6; ++n) pi[(long long)n * P.N + i.s] = v[n];
+}
+
 // sums over fluid sites of { rho, rho u_x,y,z, u_x,y,z, u_x^2,y^2,z^2 } -> acc[10] (fp64 atomics)
 template <typename real, bool WALLS>
 __global__ void __launch_bounds__(128)

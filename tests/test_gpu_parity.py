@@ -286,3 +286,13 @@ def test_bgk_model_refuses_force_and_differs_from_reg():
     reg = binding.Rflbm(8, 8, 8, 0.8, 1e-4, 1.0, 3)
     reg.init(); reg.step(20)
     assert (sim.get_populations() - reg.get_populations()).abs().max().item() > 1e-6
+
+
+@pytest.mark.parametrize("prec,walls", [(binding.F64, False), (binding.F64, True), (binding.F32, True)])
+def test_stress_observable_matches_oracle(prec, walls):
+    nx, ny, nz = 40, 9, 6
+    sim, ref = make_pair(nx, ny, nz, 0.8, 1e-4, 13, precision=prec, walls=walls, force=(1e-6, 0.0, 0.0) if walls else None)
+    init_pair(sim, ref, synthetic.smooth_random_fields(nx, ny, nz, 6))
+    sim.step(15); ref.step(15)
+    d = np.abs(sim.stress().cpu().numpy().astype(np.float64) - ref.stress()).max()
+    assert d < (1e-12 if prec == binding.F64 else 1e-5), d

@@ -150,3 +150,26 @@ def test_argument_validation():
     assert lib.rflbm_ref_set_walls_z(h, 1) == -1          # nz < 3
     assert lib.rflbm_ref_step(h, 1) == -2                  # not initialised
     lib.rflbm_ref_destroy(h)
+
+
+def test_stress_observable_is_second_hermite_moment():
+    """Pi_ab = a_0,ab + a_1,ab (Eq.18-19) = rows k=4..9 of the paper's printed basis applied to the
+    state; for an equilibrium state it is rho u_a u_b exactly (Eq.20)."""
+    from paper_tables import exact_basis
+    c, w = oracle.tables()[:2]
+    E = np.array([[float(v) for v in row] for row in exact_basis(c)])
+    nx, ny, nz = 5, 4, 6
+    f = synthetic.random_population_field(nx, ny, nz, 8, w)
+    r = oracle.Ref(nx, ny, nz, 0.8, 1e-4, 1.0, 2)
+    r.set_walls_z(True)
+    r.set_populations(f, 0)
+    pi = r.stress()
+    want = np.einsum("ki,izyx->kzyx", E[4:10], f)
+    assert np.abs(pi[:, 1:-1] - want[:, 1:-1]).max() < 1e-15
+    assert (pi[:, 0] == 0).all() and (pi[:, -1] == 0).all()           # solid layers
+    r2 = oracle.Ref(nx, ny, nz, 0.8, 0.0)
+    rho, u = synthetic.smooth_random_fields(nx, ny, nz, 3)
+    r2.init(rho, u)
+    idx = [(0, 0), (1, 1), (2, 2), (0, 1), (0, 2), (1, 2)]
+    eq = np.stack([rho * u[a] * u[b] for a, b in idx])
+    assert np.abs(r2.stress() - eq).max() < 1e-15
