@@ -48,6 +48,7 @@ def parse_args():
     p.add_argument("--precision", default="f64", choices=["f64", "f32"])
     p.add_argument("--variant", default="auto", choices=["auto", "plain", "tma"])
     p.add_argument("--model", default="reg", choices=["reg", "bgk"])
+    p.add_argument("--scheme", default="ab", choices=["ab", "aa"])
     p.add_argument("--no-e2e", action="store_true")
     p.add_argument("--no-cpu", action="store_true")
     p.add_argument("--cpu-seconds", type=float, default=12.0)
@@ -224,7 +225,8 @@ def run_ours(args):
     N = n ** 3
     K, W = args.steps, max(3, args.warmup)
 
-    sim = binding.Rflbm(n, n, n, WORKLOAD["tau"], args.kT, WORKLOAD["rho0"], WORKLOAD["seed"], prec, device=dev)
+    sim = binding.Rflbm(n, n, n, WORKLOAD["tau"], args.kT, WORKLOAD["rho0"], WORKLOAD["seed"], prec, device=dev,
+                        scheme=binding.SCHEME_AA if args.scheme == "aa" else binding.SCHEME_AB)
     sim.set_kernel_variant({"auto": binding.KERNEL_AUTO, "plain": binding.KERNEL_PLAIN, "tma": binding.KERNEL_TMA}[args.variant])
     if args.model == "bgk":
         sim.set_model(binding.MODEL_BGK)

@@ -44,7 +44,8 @@ enum { RFLBM_OK = 0, RFLBM_EINVAL = -1, RFLBM_ESTATE = -2, RFLBM_ENOMEM = -3, RF
 int rflbm_create(int nx, int ny, int nz, double tau, double kT, double rho0, uint64_t seed, int precision,
                  rflbm_t** out);
 
-/* Bytes of device workspace the handle needs: two population buffers 2*27*N*sizeof(real) (A-B scheme)
+/* Bytes of device workspace the handle needs: two population buffers 2*27*QS*sizeof(real) (A-B scheme; one for AA;
+ * QS = N rounded up to 32 plus a 9.5 KB skew for N >= 65536)
  * plus a 4 KiB reduction scratch and 12 KiB of Box-Muller tables (uploaded by rflbm_set_workspace, synchronously). */
 size_t rflbm_workspace_bytes(const rflbm_t* h);
 
@@ -71,6 +72,15 @@ int rflbm_init(rflbm_t* h, const void* rho_dev, const void* u_dev);
  * (Eq.7 :87 pull form; Eq.2-3 :56-58; Eq.19 :153; Eq.20 :160; Eq.8-9 :93-99; Eq.10 :105).
  * rflbm_step(a); rflbm_step(b) is bit-identical to rflbm_step(a+b).  ESTATE before init. */
 int rflbm_step(rflbm_t* h, int nsteps);
+
+/* Storage scheme.  RFLBM_SCHEME_AB (default): two population buffers, read one / write the other.
+ * RFLBM_SCHEME_AA: ONE buffer updated in place (half the footprint: 29 GB instead of 58 GB at 512^3 fp64, same
+ * bytes moved per step): even steps read and write the site's own 27 slots (f*_q goes to slot 26-q), odd steps
+ * read slot 26-q of x - c_q and write slot q of x + c_q; every thread writes exactly the locations it read.
+ * Results are bit-identical to the A-B scheme (same arithmetic); the observable state (R10) does not depend on it.
+ * Must be called before rflbm_set_workspace (ESTATE afterwards): rflbm_workspace_bytes depends on it. */
+enum { RFLBM_SCHEME_AB = 0, RFLBM_SCHEME_AA = 1 };
+int rflbm_set_scheme(rflbm_t* h, int scheme);
 
 /* Collision model.  RFLBM_MODEL_REG (default): the regularized fluctuating model, Eq.24, the hot
  * path.  RFLBM_MODEL_BGK: the paper's comparison model BGK-FLBM, Eq.11 (:109-111) with Eq.6 (:85): every

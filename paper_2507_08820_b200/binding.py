@@ -13,6 +13,7 @@ F64, F32 = 0, 1
 OK, EINVAL, ESTATE, ENOMEM, ECUDA = 0, -1, -2, -3, -4
 KERNEL_AUTO, KERNEL_PLAIN, KERNEL_TMA = 0, 1, 2
 MODEL_REG, MODEL_BGK = 0, 1
+SCHEME_AB, SCHEME_AA = 0, 1
 Q = 27
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -30,6 +31,7 @@ SYMBOLS = {
     "rflbm_set_force": (_i32, [_vp, _dbl, _dbl, _dbl]),
     "rflbm_set_kernel_variant": (_i32, [_vp, _i32]),
     "rflbm_set_model": (_i32, [_vp, _i32]),
+    "rflbm_set_scheme": (_i32, [_vp, _i32]),
     "rflbm_init": (_i32, [_vp, _vp, _vp]),
     "rflbm_step": (_i32, [_vp, _i32]),
     "rflbm_moments": (_i32, [_vp, _vp, _vp]),
@@ -77,7 +79,8 @@ class Rflbm:
     """One simulation handle.  Tensors are torch CUDA tensors in the x-fastest layout
     rho[nz,ny,nx], u[3,nz,ny,nx], f[27,nz,ny,nx] (canonical velocity order), dtype float64 or float32."""
 
-    def __init__(self, nx, ny, nz, tau, kT, rho0=1.0, seed=0, precision=F64, device="cuda:0", stream=None):
+    def __init__(self, nx, ny, nz, tau, kT, rho0=1.0, seed=0, precision=F64, device="cuda:0", stream=None,
+                 scheme=SCHEME_AB):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("CUDA is not available: the rflbm path has no CPU fallback")
@@ -94,6 +97,8 @@ class Rflbm:
         if rc != OK:
             raise RflbmError(rc, "rflbm_create: invalid argument")
         self.h = h
+        if scheme != SCHEME_AB:
+            self._ck(self.lib.rflbm_set_scheme(self.h, int(scheme)))
         nbytes = self.lib.rflbm_workspace_bytes(self.h)
         with torch.cuda.device(self.device):
             self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)   # owned here, borrowed by C

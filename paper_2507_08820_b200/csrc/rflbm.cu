@@ -26,6 +26,8 @@ struct rflbm {
     int precision;
     int walls;
     int model;           // RFLBM_MODEL_REG / RFLBM_MODEL_BGK
+    int scheme;          // RFLBM_SCHEME_AB (two buffers) / RFLBM_SCHEME_AA (one buffer, in place)
+    int aa_phase;        // AA: 0 = natural layout (next step is the in-place one), 1 = after an in-place step
     double g[3];
     bool force;
     void* ws;            // borrowed workspace
@@ -145,7 +147,7 @@ extern "C" int rflbm_create(int nx, int ny, int nz, double tau, double kT, doubl
 extern "C" size_t rflbm_workspace_bytes(const rflbm_t* h)
 {
     if (!h) return 0;
-    return 2 * align_up(pop_bytes(h), 256) + 4096 + TABLE_BYTES;
+    return (h->scheme == RFLBM_SCHEME_AA ? 1 : 2) * align_up(pop_bytes(h), 256) + 4096 + TABLE_BYTES;
 }
 
 extern "C" int rflbm_set_workspace(rflbm_t* h, void* dev_ptr, size_t bytes)
@@ -158,10 +160,12 @@ extern "C" int rflbm_set_workspace(rflbm_t* h, void* dev_ptr, size_t bytes)
     h->ws = dev_ptr;
     h->ws_bytes = bytes;
     const size_t pb = align_up(pop_bytes(h), 256);
+    const size_t nbuf = (h->scheme == RFLBM_SCHEME_AA) ? 1 : 2;
     h->buf[0] = dev_ptr;
-    h->buf[1] = (char*)dev_ptr + pb;
-    h->acc = (double*)((char*)dev_ptr + 2 * pb);
-    h->tables = (f64x2*)((char*)dev_ptr + 2 * pb + 4096);
+    h->buf[1] = (nbuf == 2) ? (char*)dev_ptr + pb : nullptr;
+    h->acc = (double*)((char*)dev_ptr + nbuf * pb);
+    h->tables = (f64x2*)((char*)dev_ptr + nbuf * pb + 4096);
+    h->aa_phase = 0;
     h->cur = 0;
     h->inited = false;
     if (int rc0 = check_cuda(h, cudaMemset(h->acc, 0, 4096), "scratch clear")) return rc0;
@@ -174,7 +178,7 @@ extern "C" int rflbm_set_workspace(rflbm_t* h, void* dev_ptr, size_t bytes)
     // TMA path: rows of at least one 128-site tile, row pitch a multiple of 16 bytes (nx even for fp64, nx % 4 == 0 for fp32)
     h->tma_ok = false;
     if (h->nx >= TMA_MIN_NX && h->nx % (16 / (int)real_size(h)) == 0)
-        h->tma_ok = make_tensor_map(h, h->buf[0], &h->tmap[0]) && make_tensor_map(h, h->buf[1], &h->tmap[1]);
+        h->tma_ok = make_tensor_map(h, h->buf[0], &h->tmap[0]) && (nbuf == 1 || make_tensor_map(h, h->buf[1], &h->tmap[1]));
     return RFLBM_OK;
 }
 
@@ -212,6 +216,7 @@ static FieldParams<real> field_params(const rflbm* h)
     P.nx = h->nx; P.ny = h->ny; P.nz = h->nz; P.N = h->N; P.QS = h->QS;
     P.hgx = (real)(0.5 * h->g[0]); P.hgy = (real)(0.5 * h->g[1]); P.hgz = (real)(0.5 * h->g[2]);
     P.walls = h->walls;
+    P.aa = (h->scheme == RFLBM_SCHEME_AA) ? 1 : 0;
     return P;
 }
 
@@ -242,6 +247,25 @@ static StepParams<real> step_params(const rflbm* h, uint64_t t)
     return P;
 }
 
+// which gather reads the observable state S_t out of the current buffer (rflbm_kernels.cuh)
+static int gather_mode(const rflbm* h)
+{
+    return h->scheme == RFLBM_SCHEME_AB ? GATHER_AB : (h->aa_phase ? GATHER_AA1 : GATHER_AA0);
+}
+#define RFLBM_LAUNCH_OBSERVABLE(KERNEL, ...)                                                                      \
+    do {                                                                                                          \
+        const int gm_ = gather_mode(h);                                                                           \
+        if (h->walls) {                                                                                           \
+            if (gm_ == GATHER_AB) KERNEL<real, true, GATHER_AB><<<h->grid, h->block, 0, h->stream>>>(__VA_ARGS__);       \
+            else if (gm_ == GATHER_AA1) KERNEL<real, true, GATHER_AA1><<<h->grid, h->block, 0, h->stream>>>(__VA_ARGS__); \
+            else KERNEL<real, true, GATHER_AA0><<<h->grid, h->block, 0, h->stream>>>(__VA_ARGS__);                       \
+        } else {                                                                                                  \
+            if (gm_ == GATHER_AB) KERNEL<real, false, GATHER_AB><<<h->grid, h->block, 0, h->stream>>>(__VA_ARGS__);      \
+            else if (gm_ == GATHER_AA1) KERNEL<real, false, GATHER_AA1><<<h->grid, h->block, 0, h->stream>>>(__VA_ARGS__); \
+            else KERNEL<real, false, GATHER_AA0><<<h->grid, h->block, 0, h->stream>>>(__VA_ARGS__);                      \
+        }                                                                                                         \
+    } while (0)
+
 // ---------------------------------------------------------------- init / import / export
 template <typename real>
 static int do_init(rflbm* h, const void* rho, const void* u)
@@ -264,6 +288,7 @@ extern "C" int rflbm_init(rflbm_t* h, const void* rho_dev, const void* u_dev)
     const int rc = (h->precision == RFLBM_F64) ? do_init<double>(h, rho_dev, u_dev) : do_init<float>(h, rho_dev, u_dev);
     if (rc != RFLBM_OK) return rc;
     h->cur = 0;
+    h->aa_phase = 0;
     h->t = 0;
     h->inited = true;
     return RFLBM_OK;
@@ -288,6 +313,7 @@ extern "C" int rflbm_set_populations(rflbm_t* h, const void* f_dev, uint64_t ste
     const int rc = (h->precision == RFLBM_F64) ? do_import<double>(h, f_dev) : do_import<float>(h, f_dev);
     if (rc != RFLBM_OK) return rc;
     h->cur = 0;
+    h->aa_phase = 0;
     h->t = step;
     h->inited = true;
     return RFLBM_OK;
@@ -297,10 +323,7 @@ template <typename real>
 static int do_export(rflbm* h, void* f)
 {
     const FieldParams<real> P = field_params<real>(h);
-    if (h->walls)
-        export_kernel<real, true><<<h->grid, h->block, 0, h->stream>>>((const real*)h->buf[h->cur], (real*)f, P);
-    else
-        export_kernel<real, false><<<h->grid, h->block, 0, h->stream>>>((const real*)h->buf[h->cur], (real*)f, P);
+    RFLBM_LAUNCH_OBSERVABLE(export_kernel, (const real*)h->buf[h->cur], (real*)f, P);
     return after_launch(h, "export_kernel");
 }
 
@@ -313,39 +336,49 @@ extern "C" int rflbm_get_populations(rflbm_t* h, void* f_dev)
 }
 
 // ---------------------------------------------------------------- the time step
-template <typename real, bool WALLS, bool FORCE, bool NOISE, bool BGK>
+template <typename real, bool WALLS, bool FORCE, bool NOISE, bool BGK, int PHASE>
 static void launch_one(rflbm* h, const StepParams<real>& P, bool tma)
 {
+    // A-B: read buf[cur], write the other buffer; AA: one buffer, in place
+    const real* src = (const real*)h->buf[h->cur];
+    real* dst = (real*)h->buf[PHASE == STEP_AB ? (h->cur ^ 1) : h->cur];
     if (tma) {
         const dim3 grid((h->nx + TILE_X - 1) / TILE_X, (h->ny + h->tma_rows - 1) / h->tma_rows, h->nz);
-        step_kernel_tma<real, WALLS, FORCE, NOISE, BGK><<<grid, TILE_X, 0, h->stream>>>(
-            h->tmap[h->cur], (const real*)h->buf[h->cur], (real*)h->buf[h->cur ^ 1], P, h->tma_rows);
+        step_kernel_tma<real, WALLS, FORCE, NOISE, BGK, PHASE><<<grid, TILE_X, 0, h->stream>>>(
+            h->tmap[h->cur], src, dst, P, h->tma_rows);
     } else {
-        step_kernel<real, WALLS, FORCE, NOISE, BGK>
-            <<<h->grid, h->block, 0, h->stream>>>((const real*)h->buf[h->cur], (real*)h->buf[h->cur ^ 1], P);
+        step_kernel<real, WALLS, FORCE, NOISE, BGK, PHASE><<<h->grid, h->block, 0, h->stream>>>(src, dst, P);
     }
 }
 
 static bool use_tma(const rflbm* h) { return h->tma_ok && h->variant != RFLBM_KERNEL_PLAIN; }
 
 // variant bits: 8 = BGK-FLBM, 4 = walls, 2 = force, 1 = noise (BGK carries no force: rflbm_set_model / set_force)
+template <typename real, int PHASE>
+static void dispatch_variant(rflbm* h, const StepParams<real>& P, int variant, bool tma)
+{
+    switch (variant) {
+        case 0: launch_one<real, false, false, false, false, PHASE>(h, P, tma); break;
+        case 1: launch_one<real, false, false, true, false, PHASE>(h, P, tma); break;
+        case 2: launch_one<real, false, true, false, false, PHASE>(h, P, tma); break;
+        case 3: launch_one<real, false, true, true, false, PHASE>(h, P, tma); break;
+        case 4: launch_one<real, true, false, false, false, PHASE>(h, P, tma); break;
+        case 5: launch_one<real, true, false, true, false, PHASE>(h, P, tma); break;
+        case 6: launch_one<real, true, true, false, false, PHASE>(h, P, tma); break;
+        case 7: launch_one<real, true, true, true, false, PHASE>(h, P, tma); break;
+        case 8: launch_one<real, false, false, false, true, PHASE>(h, P, tma); break;
+        case 9: launch_one<real, false, false, true, true, PHASE>(h, P, tma); break;
+        case 12: launch_one<real, true, false, false, true, PHASE>(h, P, tma); break;
+        default: launch_one<real, true, false, true, true, PHASE>(h, P, tma); break;     // 13
+    }
+}
+
 template <typename real>
 static void dispatch_step(rflbm* h, const StepParams<real>& P, int variant, bool tma)
 {
-    switch (variant) {
-        case 0: launch_one<real, false, false, false, false>(h, P, tma); break;
-        case 1: launch_one<real, false, false, true, false>(h, P, tma); break;
-        case 2: launch_one<real, false, true, false, false>(h, P, tma); break;
-        case 3: launch_one<real, false, true, true, false>(h, P, tma); break;
-        case 4: launch_one<real, true, false, false, false>(h, P, tma); break;
-        case 5: launch_one<real, true, false, true, false>(h, P, tma); break;
-        case 6: launch_one<real, true, true, false, false>(h, P, tma); break;
-        case 7: launch_one<real, true, true, true, false>(h, P, tma); break;
-        case 8: launch_one<real, false, false, false, true>(h, P, tma); break;
-        case 9: launch_one<real, false, false, true, true>(h, P, tma); break;
-        case 12: launch_one<real, true, false, false, true>(h, P, tma); break;
-        default: launch_one<real, true, false, true, true>(h, P, tma); break;     // 13
-    }
+    if (h->scheme == RFLBM_SCHEME_AB) dispatch_variant<real, STEP_AB>(h, P, variant, tma);
+    else if (h->aa_phase == 0) dispatch_variant<real, STEP_AA_EVEN>(h, P, variant, tma);
+    else dispatch_variant<real, STEP_AA_ODD>(h, P, variant, tma);
 }
 
 template <typename real>
@@ -361,7 +394,8 @@ static int do_step(rflbm* h, int nsteps)
         dispatch_step<real>(h, P, variant, tma);
         const int rc = after_launch(h, tma ? "step_kernel_tma" : "step_kernel");
         if (rc != RFLBM_OK) return rc;
-        h->cur ^= 1;
+        if (h->scheme == RFLBM_SCHEME_AB) h->cur ^= 1;
+        else h->aa_phase ^= 1;
         h->t += 1;
     }
     return RFLBM_OK;
@@ -380,10 +414,7 @@ template <typename real>
 static int do_moments(rflbm* h, void* rho, void* u)
 {
     const FieldParams<real> P = field_params<real>(h);
-    if (h->walls)
-        moments_kernel<real, true><<<h->grid, h->block, 0, h->stream>>>((const real*)h->buf[h->cur], (real*)rho, (real*)u, P);
-    else
-        moments_kernel<real, false><<<h->grid, h->block, 0, h->stream>>>((const real*)h->buf[h->cur], (real*)rho, (real*)u, P);
+    RFLBM_LAUNCH_OBSERVABLE(moments_kernel, (const real*)h->buf[h->cur], (real*)rho, (real*)u, P);
     return after_launch(h, "moments_kernel");
 }
 
@@ -399,10 +430,7 @@ template <typename real>
 static int do_stress(rflbm* h, void* pi)
 {
     const FieldParams<real> P = field_params<real>(h);
-    if (h->walls)
-        stress_kernel<real, true><<<h->grid, h->block, 0, h->stream>>>((const real*)h->buf[h->cur], (real*)pi, P);
-    else
-        stress_kernel<real, false><<<h->grid, h->block, 0, h->stream>>>((const real*)h->buf[h->cur], (real*)pi, P);
+    RFLBM_LAUNCH_OBSERVABLE(stress_kernel, (const real*)h->buf[h->cur], (real*)pi, P);
     return after_launch(h, "stress_kernel");
 }
 
@@ -418,10 +446,7 @@ template <typename real>
 static int do_diagnostics(rflbm* h)
 {
     const FieldParams<real> P = field_params<real>(h);
-    if (h->walls)
-        diagnostics_kernel<real, true><<<h->grid, h->block, 0, h->stream>>>((const real*)h->buf[h->cur], h->acc, P);
-    else
-        diagnostics_kernel<real, false><<<h->grid, h->block, 0, h->stream>>>((const real*)h->buf[h->cur], h->acc, P);
+    RFLBM_LAUNCH_OBSERVABLE(diagnostics_kernel, (const real*)h->buf[h->cur], h->acc, P);
     return after_launch(h, "diagnostics_kernel");
 }
 
@@ -510,6 +535,15 @@ extern "C" int rflbm_run_host(rflbm_t* h, const void* rho_host, const void* u_ho
     rc = check_cuda(h, cudaMemcpyAsync(u_out_host, d_u, 3 * fb, cudaMemcpyDeviceToHost, h->stream), "D2H u");
     if (rc != RFLBM_OK) return rc;
     return check_cuda(h, cudaStreamSynchronize(h->stream), "cudaStreamSynchronize");
+}
+
+extern "C" int rflbm_set_scheme(rflbm_t* h, int scheme)
+{
+    if (!h) return RFLBM_EINVAL;
+    if (scheme != RFLBM_SCHEME_AB && scheme != RFLBM_SCHEME_AA) return fail(h, RFLBM_EINVAL, "unknown scheme %d", scheme);
+    if (h->ws) return fail(h, RFLBM_ESTATE, "rflbm_set_scheme must precede rflbm_set_workspace (the workspace size depends on it)");
+    h->scheme = scheme;
+    return RFLBM_OK;
 }
 
 extern "C" int rflbm_set_model(rflbm_t* h, int model)

@@ -28,16 +28,27 @@ __device__ __forceinline__ SiteIndex my_site(int nx, int ny)
     return i;
 }
 
-// Pull-gather of the 27 pre-collision populations of a site into g[cz+1][cy+1][cx+1].
-template <typename real, bool WALLS>
+// Where the pre-collision population S_t[q](x) of a site sits in the buffer:
+//   GATHER_AB   A-B scheme: slot q of the neighbour x - c_q   (bounce-back: slot 26-q of the site itself)
+//   GATHER_AA1  AA scheme after an even (in-place) step: slot 26-q of the neighbour x - c_q (bounce-back: slot q
+//               of the site itself)
+//   GATHER_AA0  AA scheme after init / an odd step: slot q of the site itself (the natural layout)
+enum { GATHER_AB = 0, GATHER_AA1 = 1, GATHER_AA0 = 2 };
+
+// Gather of the 27 pre-collision populations of a site into g[cz+1][cy+1][cx+1].
+template <typename real, bool WALLS, int MODE = GATHER_AB>
 __device__ __forceinline__ void gather(const real* __restrict__ src, long long QS, int nx, int ny, int nz,
                                        const SiteIndex& i, real (&g)[3][3][3])
 {
+    if (MODE == GATHER_AA0) {
+#pragma unroll
+        for (int q = 0; q < Q; ++q) g[q / 9][(q / 3) % 3][q % 3] = src[(long long)q * QS + i.s];   // in-place buffer: no LDG.NC
+        return;
+    }
     // neighbour coordinates x - cx etc. with periodic wrap; index a = cx+1 reads from xs[a]
     const int xs[3] = {(i.x + 1 == nx) ? 0 : i.x + 1, i.x, (i.x == 0) ? nx - 1 : i.x - 1};
     const int ys[3] = {(i.y + 1 == ny) ? 0 : i.y + 1, i.y, (i.y == 0) ? ny - 1 : i.y - 1};
     const int zs[3] = {(i.z + 1 == nz) ? 0 : i.z + 1, i.z, (i.z == 0) ? nz - 1 : i.z - 1};
-    const long long nxy = (long long)nx * ny;
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         // with walls the fluid layers are z = 1..nz-2; x - c_q is solid iff (cz=+1 and z==1) or (cz=-1 and z==nz-2)
@@ -48,13 +59,15 @@ __device__ __forceinline__ void gather(const real* __restrict__ src, long long Q
 #pragma unroll
             for (int a = 0; a < 3; ++a) {
                 const int q = a + 3 * b + 9 * c;
-                const long long pull = (long long)q * QS + row + xs[a];
-                const long long back = (long long)(26 - q) * QS + i.s;
-                g[c][b][a] = __ldg(src + ((WALLS && bounce) ? back : pull));
+                const int slot_pull = (MODE == GATHER_AA1) ? 26 - q : q;
+                const int slot_back = (MODE == GATHER_AA1) ? q : 26 - q;
+                const long long pull = (long long)slot_pull * QS + row + xs[a];
+                const long long back = (long long)slot_back * QS + i.s;
+                const long long at = (WALLS && bounce) ? back : pull;
+                g[c][b][a] = (MODE == GATHER_AB) ? __ldg(src + at) : src[at];     // AA: the buffer is written in place
             }
         }
     }
-    (void)nxy;
 }
 
 // copy the Box-Muller tables (8 KB) from global memory (L2 resident) to shared memory; ends with a barrier
@@ -68,9 +81,49 @@ __device__ __forceinline__ void stage_tables(const f64x2* __restrict__ tab, f64x
 }
 
 // ---------------------------------------------------------------- the hot kernel: one time step
-template <typename real, bool WALLS, bool FORCE, bool NOISE, bool BGK>
+// PHASE selects the storage scheme:
+//   STEP_AB       A-B double buffer: pull from src, store to dst at the site itself
+//   STEP_AA_EVEN  AA in place (src == dst): read slot q of the site, store f*_q into slot 26-q of the site
+//   STEP_AA_ODD   AA in place: read slot 26-q of x - c_q (= f*_q streamed), store f*_q into slot q of x + c_q
+//                 (halfway bounce-back: read slot q / store slot 26-q of the site itself)
+// Every thread writes exactly the 27 locations it has read (the AA property), so in-place is race free.
+enum { STEP_AB = 0, STEP_AA_EVEN = 1, STEP_AA_ODD = 2 };
+
+template <typename real, bool WALLS, int PHASE>
+__device__ __forceinline__ void scatter(real* dst, long long QS, int nx, int ny, int nz, const SiteIndex& i,
+                                        const real (&g)[3][3][3])
+{
+    if (PHASE != STEP_AA_ODD) {
+#pragma unroll
+        for (int q = 0; q < Q; ++q)
+            __stcs(dst + (long long)((PHASE == STEP_AA_EVEN) ? 26 - q : q) * QS + i.s, g[q / 9][(q / 3) % 3][q % 3]);
+        return;
+    }
+    // push: x + c_q with periodic wrap; index a = cx+1 writes to xd[a]
+    const int xd[3] = {(i.x == 0) ? nx - 1 : i.x - 1, i.x, (i.x + 1 == nx) ? 0 : i.x + 1};
+    const int yd[3] = {(i.y == 0) ? ny - 1 : i.y - 1, i.y, (i.y + 1 == ny) ? 0 : i.y + 1};
+    const int zd[3] = {(i.z == 0) ? nz - 1 : i.z - 1, i.z, (i.z + 1 == nz) ? 0 : i.z + 1};
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        // x + c_q is solid iff (cz=-1 and z==1) or (cz=+1 and z==nz-2): the population returns to the site as 26-q
+        const bool bounce = WALLS && ((c == 0 && i.z == 1) || (c == 2 && i.z == nz - 2));
+#pragma unroll
+        for (int b = 0; b < 3; ++b) {
+            const long long row = (long long)nx * ((long long)yd[b] + (long long)ny * (long long)zd[c]);
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                const int q = a + 3 * b + 9 * c;
+                const long long push = (long long)q * QS + row + xd[a];
+                const long long back = (long long)(26 - q) * QS + i.s;
+                __stcs(dst + ((WALLS && bounce) ? back : push), g[c][b][a]);
+            }
+        }
+    }
+}
+
+template <typename real, bool WALLS, bool FORCE, bool NOISE, bool BGK, int PHASE>
 __global__ void __launch_bounds__(128)
-step_kernel(const real* __restrict__ src, real* __restrict__ dst, const __grid_constant__ StepParams<real> P)
+step_kernel(const real* src, real* dst, const __grid_constant__ StepParams<real> P)
 {
     constexpr bool TABLES = NOISE && sizeof(real) == 8;
     __shared__ f64x2 s_tab[TABLES ? LOG_TABLE_N + SC_TABLE_N : 1];
@@ -79,14 +132,10 @@ step_kernel(const real* __restrict__ src, real* __restrict__ dst, const __grid_c
     if (!i.valid) return;
     if (WALLS && (i.z == 0 || i.z == P.nz - 1)) return;    // solid layers are never updated
     real g[3][3][3];
-    gather<real, WALLS>(src, P.QS, P.nx, P.ny, P.nz, i, g);
+    gather<real, WALLS, PHASE == STEP_AB ? GATHER_AB : PHASE == STEP_AA_EVEN ? GATHER_AA0 : GATHER_AA1>(
+        src, P.QS, P.nx, P.ny, P.nz, i, g);
     collide<real, FORCE, NOISE, BGK>(g, P, (uint32_t)i.s, s_tab, s_tab + LOG_TABLE_N);
-#pragma unroll
-    for (int c = 0; c < 3; ++c)
-#pragma unroll
-        for (int b = 0; b < 3; ++b)
-#pragma unroll
-            for (int a = 0; a < 3; ++a) __stcs(dst + (long long)(a + 3 * b + 9 * c) * P.QS + i.s, g[c][b][a]);
+    scatter<real, WALLS, PHASE>(dst, P.QS, P.nx, P.ny, P.nz, i, g);
 }
 
 // ---------------------------------------------------------------- observables
@@ -97,9 +146,10 @@ struct FieldParams {
     long long QS;         // elements between consecutive population arrays of the internal storage (>= N)
     real hgx, hgy, hgz;   // g/2: reported velocity u = j/rho + g/2 (R13)
     int walls;
+    int aa;               // AA scheme: one buffer in the natural layout P[q](s) = S[q](s) at even phase
 };
 
-template <typename real, bool WALLS>
+template <typename real, bool WALLS, int MODE>
 __global__ void __launch_bounds__(128)
 moments_kernel(const real* __restrict__ src, real* __restrict__ rho, real* __restrict__ u, const FieldParams<real> P)
 {
@@ -110,7 +160,7 @@ moments_kernel(const real* __restrict__ src, real* __restrict__ rho, real* __res
         return;
     }
     real g[3][3][3];
-    gather<real, WALLS>(src, P.QS, P.nx, P.ny, P.nz, i, g);
+    gather<real, WALLS, MODE>(src, P.QS, P.nx, P.ny, P.nz, i, g);
     const Moments10<real> m = forward_moments(g);
     const real inv = real(1.0) / m.rho;
     rho[i.s] = m.rho;
@@ -121,7 +171,7 @@ moments_kernel(const real* __restrict__ src, real* __restrict__ rho, real* __res
 
 // Pi_ab = sum_i f_i (c_a c_b - delta_ab/3) of the current state (Eq.18 + Eq.19):
 // pi[6][N] in the order xx, yy, zz, xy, xz, yz.  Solid nodes: 0.
-template <typename real, bool WALLS>
+template <typename real, bool WALLS, int MODE>
 __global__ void __launch_bounds__(128)
 stress_kernel(const real* __restrict__ src, real* __restrict__ pi, const FieldParams<real> P)
 {
@@ -130,7 +180,7 @@ stress_kernel(const real* __restrict__ src, real* __restrict__ pi, const FieldPa
     real v[6] = {real(0), real(0), real(0), real(0), real(0), real(0)};
     if (!(WALLS && (i.z == 0 || i.z == P.nz - 1))) {
         real g[3][3][3];
-        gather<real, WALLS>(src, P.QS, P.nx, P.ny, P.nz, i, g);
+        gather<real, WALLS, MODE>(src, P.QS, P.nx, P.ny, P.nz, i, g);
         const Moments10<real> m = forward_moments(g);
         const real third = m.rho * real(1.0 / 3.0);
         v[0] = m.pxx - third; v[1] = m.pyy - third; v[2] = m.pzz - third;
@@ -141,7 +191,7 @@ stress_kernel(const real* __restrict__ src, real* __restrict__ pi, const FieldPa
 }
 
 // sums over fluid sites of { rho, rho u_x,y,z, u_x,y,z, u_x^2,y^2,z^2 } -> acc[10] (fp64 atomics)
-template <typename real, bool WALLS>
+template <typename real, bool WALLS, int MODE>
 __global__ void __launch_bounds__(128)
 diagnostics_kernel(const real* __restrict__ src, double* __restrict__ acc, const FieldParams<real> P)
 {
@@ -152,7 +202,7 @@ diagnostics_kernel(const real* __restrict__ src, double* __restrict__ acc, const
     const bool fluid = i.valid && !(WALLS && (i.z == 0 || i.z == P.nz - 1));
     if (fluid) {
         real g[3][3][3];
-        gather<real, WALLS>(src, P.QS, P.nx, P.ny, P.nz, i, g);
+        gather<real, WALLS, MODE>(src, P.QS, P.nx, P.ny, P.nz, i, g);
         const Moments10<real> m = forward_moments(g);
         const double rho = (double)m.rho;
         const double ux = (double)m.jx / rho + (double)P.hgx;
@@ -182,7 +232,7 @@ diagnostics_kernel(const real* __restrict__ src, double* __restrict__ acc, const
 
 // ---------------------------------------------------------------- state import / export (R10)
 // out[canonical i][s] = S_t[i](s): the same gather as the step; solid nodes export their stored values.
-template <typename real, bool WALLS>
+template <typename real, bool WALLS, int MODE>
 __global__ void __launch_bounds__(128)
 export_kernel(const real* __restrict__ src, real* __restrict__ out, const FieldParams<real> P)
 {
@@ -194,7 +244,7 @@ export_kernel(const real* __restrict__ src, real* __restrict__ out, const FieldP
         return;
     }
     real g[3][3][3];
-    gather<real, WALLS>(src, P.QS, P.nx, P.ny, P.nz, i, g);
+    gather<real, WALLS, MODE>(src, P.QS, P.nx, P.ny, P.nz, i, g);
 #pragma unroll
     for (int n = 0; n < Q; ++n)
         out[(long long)n * P.N + i.s] = g[canon_cz(n) + 1][canon_cy(n) + 1][canon_cx(n) + 1];
@@ -202,6 +252,7 @@ export_kernel(const real* __restrict__ src, real* __restrict__ out, const FieldP
 
 // P[q](s) = S[q](s + c_q), or S[26-q](s) when s + c_q is solid; solid nodes store S[q](s) unchanged.
 // `in` is canonical; written to both A and B buffers so that the never-updated solid layers agree.
+// AA scheme (P.aa): the natural layout P[q](s) = S[q](s), one buffer (bufB == nullptr).
 template <typename real, bool WALLS>
 __global__ void __launch_bounds__(128)
 import_kernel(const real* __restrict__ in, real* __restrict__ bufA, real* __restrict__ bufB, const FieldParams<real> P)
@@ -214,7 +265,7 @@ import_kernel(const real* __restrict__ in, real* __restrict__ bufA, real* __rest
         const int cx = canon_cx(n), cy = canon_cy(n), cz = canon_cz(n);
         const int q = lex_of(cx, cy, cz);
         long long from = (long long)n * P.N + i.s;
-        if (!solid) {
+        if (!solid && !P.aa) {
             const int zd = i.z + cz;
             if (WALLS && (zd == 0 || zd == P.nz - 1)) {
                 // s + c_q solid: this slot is pulled back by the site itself as direction opp(q)
@@ -227,15 +278,18 @@ import_kernel(const real* __restrict__ in, real* __restrict__ bufA, real* __rest
         }
         const real v = in[from];
         bufA[(long long)q * P.QS + i.s] = v;
-        bufB[(long long)q * P.QS + i.s] = v;
+        if (bufB != nullptr) bufB[(long long)q * P.QS + i.s] = v;
     }
 }
 
 // equilibrium f^(0)_q(rho,u) in the product form of Eq.25 with Eq.20 (w_i and the Hermite sum factorise):
 //   f0 = rho phi(cx,ux) phi(cy,uy) phi(cz,uz),  phi(0,u) = 2/3 - u^2,  phi(+-1,u) = 1/6 +- u/2 + u^2/2
+// Written with explicit round-to-nearest intrinsics: the compiler must not contract or reassociate differently in
+// the A-B and AA code paths of init_kernel (the two schemes are required to agree bit for bit).
 __device__ __forceinline__ double phi1d(int c, double u)
 {
-    return (c == 0) ? (2.0 / 3.0 - u * u) : (1.0 / 6.0 + 0.5 * (double)c * u + 0.5 * u * u);
+    if (c == 0) return __fma_rn(-u, u, 2.0 / 3.0);
+    return __fma_rn(0.5 * u, __dadd_rn(u, (double)c), 1.0 / 6.0);      // 1/6 + u (u + c) / 2
 }
 
 // init (R9, R10): P_{-1}[q](s) = f0_q(rho,u)(s + c_q), or f0_{26-q}(rho,u)(s) when s + c_q is solid.
@@ -252,7 +306,7 @@ init_kernel(const real* __restrict__ rho, const real* __restrict__ u, double rho
     for (int q = 0; q < Q; ++q) {
         int cx = q % 3 - 1, cy = (q / 3) % 3 - 1, cz = q / 9 - 1;
         long long s = i.s;
-        if (!solid) {
+        if (!solid && !P.aa) {
             const int zd = i.z + cz;
             if (WALLS && (zd == 0 || zd == P.nz - 1)) {
                 cx = -cx; cy = -cy; cz = -cz;              // f0 of the opposite direction at the site itself
@@ -265,9 +319,9 @@ init_kernel(const real* __restrict__ rho, const real* __restrict__ u, double rho
         if (rho != nullptr) {
             r = (double)rho[s]; ux = (double)u[s]; uy = (double)u[P.N + s]; uz = (double)u[2 * P.N + s];
         }
-        const real v = (real)(r * phi1d(cx, ux) * phi1d(cy, uy) * phi1d(cz, uz));
+        const real v = (real)__dmul_rn(__dmul_rn(__dmul_rn(r, phi1d(cx, ux)), phi1d(cy, uy)), phi1d(cz, uz));
         bufA[(long long)q * P.QS + i.s] = v;
-        bufB[(long long)q * P.QS + i.s] = v;
+        if (bufB != nullptr) bufB[(long long)q * P.QS + i.s] = v;
     }
 }
 

@@ -86,7 +86,10 @@ __device__ __forceinline__ bool elect_one()
 }
 
 // issue the 9 box copies of the tile (x0, y, z); one thread
-template <typename real, bool WALLS>
+// PHASE (rflbm_kernels.cuh): STEP_AB pulls slot q of the neighbour row (bounce-back: slot 26-q of the own row);
+// STEP_AA_EVEN reads slot q of the own row; STEP_AA_ODD pulls slot 26-q of the neighbour row (bounce-back: slot q of
+// the own row).  A box holds three consecutive slots, so "26-q" boxes start at 24-3b-9c and hold the rows reversed.
+template <typename real, bool WALLS, int PHASE>
 __device__ __forceinline__ void issue_tile(const CUtensorMap* tmap, uint32_t s_in, uint32_t bar, int x0, int y, int z,
                                            int ny, int nz)
 {
@@ -102,16 +105,20 @@ __device__ __forceinline__ void issue_tile(const CUtensorMap* tmap, uint32_t s_i
 #pragma unroll
         for (int b = 0; b < 3; ++b) {
             const uint32_t dst = s_in + (uint32_t)((3 * c + b) * G::BOX_PITCH_BYTES);
-            if (WALLS && bounce) tma_load_box(dst, tmap, x0 - G::HALO, y, z, 24 - 3 * b - 9 * c, bar);
-            else tma_load_box(dst, tmap, x0 - G::HALO, ys[b], zs[c], 3 * b + 9 * c, bar);
+            constexpr int fwd = 0, rev = 1;
+            const int q_fwd = 3 * b + 9 * c, q_rev = 24 - 3 * b - 9 * c;
+            (void)fwd; (void)rev;
+            if (PHASE == STEP_AA_EVEN) tma_load_box(dst, tmap, x0 - G::HALO, y, z, q_fwd, bar);
+            else if (WALLS && bounce) tma_load_box(dst, tmap, x0 - G::HALO, y, z, PHASE == STEP_AB ? q_rev : q_fwd, bar);
+            else tma_load_box(dst, tmap, x0 - G::HALO, ys[b], zs[c], PHASE == STEP_AB ? q_fwd : q_rev, bar);
         }
     }
 }
 
 // fp64: 128 registers, 41 KB -> 4 blocks per SM; fp32: 64 registers, 15 KB -> 8 blocks per SM
-template <typename real, bool WALLS, bool FORCE, bool NOISE, bool BGK>
+template <typename real, bool WALLS, bool FORCE, bool NOISE, bool BGK, int PHASE>
 __global__ void __launch_bounds__(TILE_X, sizeof(real) == 8 ? 4 : 8)
-step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const real* __restrict__ src, real* __restrict__ dst,
+step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const real* src, real* dst,
                 const __grid_constant__ StepParams<real> P, int rows)
 {
     using G = TmaGeom<real>;
@@ -132,7 +139,7 @@ step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const real* __rest
     if (warp == 0 && elect_one()) {
         mbar_init(bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        issue_tile<real, WALLS>(&tmap_src, in0, bar, x0, y_begin, z, P.ny, P.nz);
+        issue_tile<real, WALLS, PHASE>(&tmap_src, in0, bar, x0, y_begin, z, P.ny, P.nz);
     }
     if (TABLES) stage_tables(P.tables, s_tab);                  // ends with __syncthreads()
     else __syncthreads();                                       // mbarrier init visible to every waiter
@@ -151,7 +158,7 @@ step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const real* __rest
         const long long s = (long long)x + (long long)P.nx * y + nxy * z;
         // periodic wrap in x: TMA zero-fills these 9 values; fetch them early, use them after the barrier
         real wv[3][3];
-        if (edge_warp) {                                        // warp-uniform branch: interior warps skip all of this
+        if (PHASE != STEP_AA_EVEN && edge_warp) {               // warp-uniform branch: interior warps skip all of this
             if (wrap_lo || wrap_hi) {
                 const int ysr[3] = {(y + 1 == P.ny) ? 0 : y + 1, y, (y == 0) ? P.ny - 1 : y - 1};
                 const int zsr[3] = {(z + 1 == P.nz) ? 0 : z + 1, z, (z == 0) ? P.nz - 1 : z - 1};
@@ -161,9 +168,10 @@ step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const real* __rest
                     for (int b = 0; b < 3; ++b) {
                         const long long row = (long long)P.nx * ysr[b] + nxy * zsr[c];
                         // x+1 -> 0 for cx = -1 (a = 0); x-1 -> nx-1 for cx = +1 (a = 2); nx >= 128 here
-                        const long long at = wrap_hi ? (long long)(0 + 3 * b + 9 * c) * P.QS + row
-                                                     : (long long)(2 + 3 * b + 9 * c) * P.QS + row + (P.nx - 1);
-                        wv[c][b] = __ldg(src + at);
+                        const int qa = (wrap_hi ? 0 : 2) + 3 * b + 9 * c;
+                        const int slot = (PHASE == STEP_AB) ? qa : 26 - qa;
+                        const long long at = (long long)slot * P.QS + row + (wrap_hi ? 0 : P.nx - 1);
+                        wv[c][b] = (PHASE == STEP_AB) ? __ldg(src + at) : src[at];   // AA: the buffer is written in place
                     }
             }
         }
@@ -176,10 +184,22 @@ step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const real* __rest
 #pragma unroll
             for (int b = 0; b < 3; ++b) {
                 const real* box = tile + (3 * c + b) * G::BOX_PITCH;
-                if (WALLS && bounce) {       // rows hold q' = 26-q in ascending q': row 2-a, the site itself at tid+HALO
+                // forward boxes hold slots q in rows a = 0,1,2; reversed boxes hold q' = 26-q in ascending q': row 2-a.
+                // Pulled rows are read with the x shift -cx, local ones (bounce-back, even AA phase) at tid+HALO.
+                const bool local = (PHASE == STEP_AA_EVEN) || (WALLS && bounce);
+                const bool reversed = (PHASE == STEP_AB) ? (WALLS && bounce) : (PHASE == STEP_AA_ODD && !(WALLS && bounce));
+                if (local && reversed) {
                     g[c][b][0] = box[2 * G::BOX_X + G::HALO];
                     g[c][b][1] = box[1 * G::BOX_X + G::HALO];
                     g[c][b][2] = box[0 * G::BOX_X + G::HALO];
+                } else if (local) {
+                    g[c][b][0] = box[0 * G::BOX_X + G::HALO];
+                    g[c][b][1] = box[1 * G::BOX_X + G::HALO];
+                    g[c][b][2] = box[2 * G::BOX_X + G::HALO];
+                } else if (reversed) {
+                    g[c][b][0] = box[2 * G::BOX_X + G::HALO + 1];
+                    g[c][b][1] = box[1 * G::BOX_X + G::HALO];
+                    g[c][b][2] = box[0 * G::BOX_X + G::HALO - 1];
                 } else {
                     g[c][b][0] = box[0 * G::BOX_X + G::HALO + 1];
                     g[c][b][1] = box[1 * G::BOX_X + G::HALO];
@@ -188,9 +208,9 @@ step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const real* __rest
             }
         }
         __syncthreads();                                       // the tile is in registers: the stage is free
-        if (warp == 0 && y + 1 < y_end && elect_one()) issue_tile<real, WALLS>(&tmap_src, in0, bar, x0, y + 1, z, P.ny, P.nz);
+        if (warp == 0 && y + 1 < y_end && elect_one()) issue_tile<real, WALLS, PHASE>(&tmap_src, in0, bar, x0, y + 1, z, P.ny, P.nz);
 
-        if (edge_warp) {
+        if (PHASE != STEP_AA_EVEN && edge_warp) {
             if (wrap_lo || wrap_hi) {
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
@@ -206,18 +226,28 @@ step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const real* __rest
         }
         if (active) {
             collide<real, FORCE, NOISE, BGK>(g, P, (uint32_t)s, s_tab, s_tab + LOG_TABLE_N);
-            const unsigned long long out = reinterpret_cast<unsigned long long>(dst + s);
+            if (PHASE == STEP_AA_ODD) {
+                // push to the neighbours x + c_q (slot q), misaligned by one element for cx = +-1: the partial
+                // sectors at the ends of a warp's 256 bytes are completed in L2 by the neighbouring warp's store
+                SiteIndex i;
+                i.x = x; i.y = y; i.z = z; i.valid = true; i.s = s;
+                scatter<real, WALLS, STEP_AA_ODD>(dst, P.QS, P.nx, P.ny, P.nz, i, g);
+            } else {
+                const unsigned long long out = reinterpret_cast<unsigned long long>(dst + s);
 #pragma unroll
-            for (int c = 0; c < 3; ++c)
+                for (int c = 0; c < 3; ++c)
 #pragma unroll
-                for (int b = 0; b < 3; ++b)
+                    for (int b = 0; b < 3; ++b)
 #pragma unroll
-                    for (int a = 0; a < 3; ++a) {
-                        // one IMAD.WIDE.U32 per store: out + QS * sizeof(real) * q (QS < 2^32, so the 32x32->64 product is exact)
-                        unsigned long long at;
-                        asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(at) : "r"(QS32), "r"((unsigned)sizeof(real) * (a + 3 * b + 9 * c)), "l"(out));
-                        __stcs(reinterpret_cast<real*>(at), g[c][b][a]);
-                    }
+                        for (int a = 0; a < 3; ++a) {
+                            // one IMAD.WIDE.U32 per store: out + QS * sizeof(real) * slot (QS < 2^32: exact 32x32->64)
+                            const int q = a + 3 * b + 9 * c;
+                            const unsigned slot = (PHASE == STEP_AA_EVEN) ? 26 - q : q;
+                            unsigned long long at;
+                            asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(at) : "r"(QS32), "r"((unsigned)sizeof(real) * slot), "l"(out));
+                            __stcs(reinterpret_cast<real*>(at), g[c][b][a]);
+                        }
+            }
         }
     }
 }

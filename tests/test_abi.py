@@ -48,6 +48,13 @@ def test_create_validation_and_workspace_size(lib):
     assert lib.rflbm_set_workspace(h, 0x1000, 16) == binding.ENOMEM
     assert lib.rflbm_set_workspace(h, 0x1001, 1 << 30) == binding.ENOMEM      # misaligned
     assert lib.rflbm_set_force(h, float("inf"), 0.0, 0.0) == binding.EINVAL
+    assert lib.rflbm_set_scheme(h, 7) == binding.EINVAL
+    assert lib.rflbm_set_scheme(h, binding.SCHEME_AA) == binding.OK
+    assert lib.rflbm_workspace_bytes(h) == 27 * 4096 * 8 + 4096 + 12288          # one buffer
+    assert lib.rflbm_set_scheme(h, binding.SCHEME_AB) == binding.OK
+    assert lib.rflbm_set_model(h, 9) == binding.EINVAL and lib.rflbm_set_model(h, binding.MODEL_BGK) == binding.OK
+    assert lib.rflbm_set_force(h, 1e-6, 0.0, 0.0) == binding.EINVAL              # BGK-FLBM carries no force
+    assert lib.rflbm_set_model(h, binding.MODEL_REG) == binding.OK
     assert lib.rflbm_step_count(h) == 0 and lib.rflbm_launch_count(h) == 0
     assert lib.rflbm_destroy(h) == binding.OK
     h32 = C.c_void_p()

@@ -296,3 +296,76 @@ def test_stress_observable_matches_oracle(prec, walls):
     sim.step(15); ref.step(15)
     d = np.abs(sim.stress().cpu().numpy().astype(np.float64) - ref.stress()).max()
     assert d < (1e-12 if prec == binding.F64 else 1e-5), d
+
+
+@pytest.mark.parametrize("shape,prec,walls,force,kT,variant", [
+    ((16, 16, 16), binding.F64, False, None, 1e-4, binding.KERNEL_AUTO),
+    ((5, 7, 9), binding.F64, True, (1e-5, -2e-6, 3e-6), 1e-4, binding.KERNEL_AUTO),
+    ((33, 6, 5), binding.F32, True, (1e-6, 0.0, 0.0), 1e-4, binding.KERNEL_AUTO),
+    ((1, 1, 1), binding.F64, False, None, 1e-4, binding.KERNEL_AUTO),
+    ((130, 18, 5), binding.F64, True, (1e-5, 2e-6, -3e-6), 1e-4, binding.KERNEL_TMA),
+    ((256, 20, 3), binding.F64, False, None, 1e-4, binding.KERNEL_TMA),
+    ((300, 3, 4), binding.F64, False, None, 0.0, binding.KERNEL_TMA),
+    ((136, 5, 6), binding.F32, True, None, 1e-4, binding.KERNEL_TMA),
+    ((256, 4, 3), binding.F64, False, None, 1e-4, binding.KERNEL_PLAIN)])
+def test_aa_in_place_scheme_is_bit_identical_to_ab_and_matches_oracle(shape, prec, walls, force, kT, variant):
+    """AA (one buffer, in place) against A-B: same arithmetic, so bit-identical observable state after even AND
+    odd step counts (the export gathers differently in the two AA phases), moments and stress included."""
+    torch = torch_()
+    nx, ny, nz = shape
+    fields = synthetic.smooth_random_fields(nx, ny, nz, 31)
+    sims = {}
+    for scheme in (binding.SCHEME_AB, binding.SCHEME_AA):
+        sim = binding.Rflbm(nx, ny, nz, 0.8, kT, 1.0, 37, prec, scheme=scheme)
+        if walls:
+            sim.set_walls_z(True)
+        if force is not None:
+            sim.set_force(*force)
+        sim.set_kernel_variant(variant)
+        sim.init(torch.from_numpy(fields[0]), torch.from_numpy(fields[1]))
+        sims[scheme] = sim
+    ab, aa = sims[binding.SCHEME_AB], sims[binding.SCHEME_AA]
+    assert aa.workspace.numel() < 0.52 * ab.workspace.numel() + 40000
+    assert torch.equal(ab.get_populations(), aa.get_populations())
+    ref = oracle.Ref(nx, ny, nz, 0.8, kT, 1.0, 37, prec, threads=NT)
+    if walls:
+        ref.set_walls_z(True)
+    if force is not None:
+        ref.set_force(*force)
+    ref.init(*fields)
+    for n in (1, 1, 5, 12, 21):                       # odd and even totals: 1, 2, 7, 19, 40
+        ab.step(n); aa.step(n); ref.step(n)
+        assert torch.equal(ab.get_populations(), aa.get_populations()), ab.step_count
+        ra, ua = aa.moments(); rb, ub = ab.moments()
+        assert torch.equal(ra, rb) and torch.equal(ua, ub) and torch.equal(aa.stress(), ab.stress())
+        assert np.allclose(aa.diagnostics(), ab.diagnostics(), rtol=1e-12, atol=1e-12)   # atomics: order varies
+    err = np.abs(aa.get_populations().cpu().numpy().astype(np.float64) - ref.get_populations()).max()
+    assert err < (TOL64 if prec == binding.F64 else TOL32), err
+
+
+def test_aa_set_get_roundtrip_resume_and_bgk():
+    torch = torch_()
+    w = oracle.tables()[1]
+    nx, ny, nz = 9, 6, 5
+    f = synthetic.random_population_field(nx, ny, nz, 4, w)
+    for walls in (False, True):
+        sim = binding.Rflbm(nx, ny, nz, 0.8, 1e-4, 1.0, 11, scheme=binding.SCHEME_AA)
+        ref = oracle.Ref(nx, ny, nz, 0.8, 1e-4, 1.0, 11, threads=NT)
+        if walls:
+            sim.set_walls_z(True); ref.set_walls_z(True)
+        sim.set_populations(torch.from_numpy(f), 17); ref.set_populations(f, 17)
+        assert np.array_equal(pops(sim), f)
+        sim.step(7); ref.step(7)                      # odd phase
+        assert np.abs(pops(sim) - ref.get_populations()).max() < TOL64
+        mid = sim.get_populations().clone()
+        sim.step(6); ref.step(6)
+        assert np.abs(pops(sim) - ref.get_populations()).max() < TOL64
+        # resume from the odd-phase export in a fresh handle: bit exact
+        sim2 = binding.Rflbm(nx, ny, nz, 0.8, 1e-4, 1.0, 11, scheme=binding.SCHEME_AA)
+        if walls:
+            sim2.set_walls_z(True)
+        sim2.set_populations(mid, 24); sim2.step(6)
+        assert torch.equal(sim2.get_populations(), sim.get_populations())
+    a = binding.Rflbm(20, 8, 6, 0.7, 1e-4, 1.0, 3, scheme=binding.SCHEME_AA); a.set_model(binding.MODEL_BGK); a.init(); a.step(15)
+    b = binding.Rflbm(20, 8, 6, 0.7, 1e-4, 1.0, 3); b.set_model(binding.MODEL_BGK); b.init(); b.step(15)
+    assert torch.equal(a.get_populations(), b.get_populations())
