@@ -73,6 +73,8 @@ def load():
     lib.rflbm_ref_collide_site.argtypes = [pd, dbl, dbl, u64, i32, pd, C.c_uint32, u64, pd]
     lib.rflbm_ref_collide_site_bgk.argtypes = [pd, dbl, dbl, u64, i32, C.c_uint32, u64, pd]
     lib.rflbm_ref_set_model.argtypes = [vp, i32]
+    lib.rflbm_ref_set_ghost_tau.argtypes = [vp, dbl]
+    lib.rflbm_ref_collide_site_ghost.argtypes = [pd, dbl, dbl, dbl, u64, i32, C.c_uint32, u64, pd]
     lib.rflbm_ref_moments_of.argtypes = [pd, pd]
     lib.rflbm_ref_moments_of.restype = None
     _lib = lib
@@ -118,6 +120,14 @@ def collide_site(g, tau, kT=0.0, seed=0, precision=F64, gacc=(0.0, 0.0, 0.0), si
     out = np.zeros(Q)
     load().rflbm_ref_collide_site(np.ascontiguousarray(g, np.float64), float(tau), float(kT), int(seed),
                                   precision, np.ascontiguousarray(gacc, np.float64), int(site), int(t), out)
+    return out
+
+
+def collide_site_ghost(g, tau, tau_g, kT=0.0, seed=0, precision=F64, site=0, t=0):
+    """Reg-FLBM collision with a general ghost relaxation time (Eq.21 live)."""
+    out = np.zeros(Q)
+    load().rflbm_ref_collide_site_ghost(np.ascontiguousarray(g, np.float64), float(tau), float(tau_g), float(kT),
+                                        int(seed), precision, int(site), int(t), out)
     return out
 
 
@@ -168,6 +178,9 @@ class Ref:
 
     def set_walls_z(self, on=True):
         self._ck(self.lib.rflbm_ref_set_walls_z(self.h, int(on)), "set_walls_z")
+
+    def set_ghost_tau(self, tau_g):
+        self._ck(self.lib.rflbm_ref_set_ghost_tau(self.h, float(tau_g)), "set_ghost_tau")
 
     def set_model(self, model):
         self._ck(self.lib.rflbm_ref_set_model(self.h, int(model)), "set_model")

@@ -18,6 +18,7 @@
  *   noise phi_k r_k, k=4..26     :93-99   Eq.8-9 (k=1..3 carry no noise, :95; R3)
  *   back-transform               :105     Eq.10 (== Eq.25+26, :225-229)
  *   final update                 :221     Eq.24  with omega_g = 1 (:215)
+ *   general ghost rate omega_g   :163-166 Eq.21 recursion (perm: DESIGN.md R20), :211-215
  *   BGK-FLBM (comparison model)  :109-111 Eq.11 with Eq.6 (:85), in population space (f^eq: DESIGN.md R19)
  *   streaming                    :87      Eq.7   (periodic; bounce-back walls: DESIGN.md R12)
  *   body force (Guo, moment form): not in the paper, R13
@@ -218,6 +219,7 @@ typedef struct rflbm_ref {
     int precision;
     int walls_z;
     int model;    /* REF_MODEL_REG (Eq.24) or REF_MODEL_BGK (Eq.11) */
+    double tau_g; /* ghost relaxation time 1/omega_g of Reg-FLBM; 0 or 1 = the paper's choice omega_g = 1 (:215) */
     double g[3];
     uint64_t t;
     int inited;
@@ -248,6 +250,7 @@ int rflbm_ref_create(int nx, int ny, int nz, double tau, double kT, double rho0,
     h->nx = nx; h->ny = ny; h->nz = nz;
     h->tau = tau; h->kT = kT; h->rho0 = rho0; h->seed = seed; h->precision = precision;
     h->nthreads = 1;
+    h->tau_g = 1.0;
     size_t n = nsites(h);
     h->S = (double *)malloc(sizeof(double) * Q * n);
     h->S2 = (double *)malloc(sizeof(double) * Q * n);
@@ -292,6 +295,13 @@ int rflbm_ref_set_force(rflbm_ref_t *h, double gx, double gy, double gz)
     if (!h || !isfinite(gx) || !isfinite(gy) || !isfinite(gz)) return REF_EINVAL;
     if (h->model == REF_MODEL_BGK && (gx != 0.0 || gy != 0.0 || gz != 0.0)) return REF_EINVAL;
     h->g[0] = gx; h->g[1] = gy; h->g[2] = gz;
+    return REF_OK;
+}
+
+int rflbm_ref_set_ghost_tau(rflbm_ref_t *h, double tau_g)
+{
+    if (!h || !isfinite(tau_g) || !(tau_g > 0.5)) return REF_EINVAL;
+    h->tau_g = tau_g;
     return REF_OK;
 }
 
@@ -349,6 +359,49 @@ int rflbm_ref_init(rflbm_ref_t *h, const double *rho, const double *u)
 
 /* ------------------------------------------------------------------ collision at one site */
 
+/* Eq.21, the recursive non-equilibrium Hermite coefficients of order n >= 3, literally:
+ *   a1^(n)[a1..an] = a1^(n-1)[a1..a(n-1)] u[an] + ( u[a1]..u[a(n-2)] a1^(2)[a(n-1) an] + perm(an) ),
+ * "perm(an)" = the permutations that pair an with each of the first n-1 indices in turn (reading R20: these are
+ * the n-1 terms sum_j a1^(2)[aj an] prod_{k<n, k!=j} u[ak]; Malaspinas' recursive regularization, ref. 55).
+ * Tensors of rank n are stored with 3^n entries, index = a1 3^(n-1) + ... + an.  A[2] is the input a1^(2). */
+static void a1_recursion(const double a2[3][3], const double u[3], double A3[27], double A4[81], double A5[243],
+                         double A6[729])
+{
+    double A2[9];
+    for (int i = 0; i < 3; i++)
+        for (int j = 0; j < 3; j++) A2[3 * i + j] = a2[i][j];
+    double *A[7] = {0, 0, A2, A3, A4, A5, A6};
+    int size = 9;
+    for (int n = 3; n <= 6; n++) {
+        size *= 3;
+        for (int idx = 0; idx < size; idx++) {
+            int al[6], t = idx;
+            for (int k = n - 1; k >= 0; k--) { al[k] = t % 3; t /= 3; }       /* al[0..n-1] = a1..an */
+            double val = A[n - 1][idx / 3] * u[al[n - 1]];
+            for (int j = 0; j < n - 1; j++) {
+                double term = a2[al[j]][al[n - 1]];
+                for (int k = 0; k < n - 1; k++)
+                    if (k != j) term *= u[al[k]];
+                val += term;
+            }
+            A[n][idx] = val;
+        }
+    }
+}
+
+/* coefficient of mode k = (p,q,r): the tensor entry with p x-indices, q y-indices, r z-indices (any order) */
+static double a1_of_mode(int k, const double a2[3][3], const double A3[27], const double A4[81], const double A5[243],
+                         const double A6[729])
+{
+    int al[6], n = 0;
+    for (int a = 0; a < 3; a++)
+        for (int m = 0; m < T_pqr[k][a]; m++) al[n++] = a;
+    int idx = 0;
+    for (int m = 0; m < n; m++) idx = 3 * idx + al[m];
+    if (n == 2) return a2[al[0]][al[1]];
+    return (n == 3) ? A3[idx] : (n == 4) ? A4[idx] : (n == 5) ? A5[idx] : A6[idx];
+}
+
 /* steps 2-7 of DESIGN.md "one step"; g = pre-collision populations of the site */
 static void collide(const rflbm_ref_t *h, const double g[Q], uint32_t site, uint64_t t, double fstar[Q])
 {
@@ -388,6 +441,15 @@ static void collide(const rflbm_ref_t *h, const double g[Q], uint32_t site, uint
 
     /* 5. relaxed hydrodynamic non-equilibrium part, Eq.26 with (1-omega_h), Eq.24; ghosts: 1-omega_g = 0 */
     for (int m = 0; m < 6; m++) M[4 + m] += (1.0 - omega_h) * a1[m];
+    /* general ghost rate (:211-215 before omega_g is set to 1): (1-omega_g) f^(1,g), the ghost part of Eq.17 with
+     * the coefficients of Eq.21 */
+    const double omega_g = (h->tau_g > 0.0) ? 1.0 / h->tau_g : 1.0;
+    if (omega_g != 1.0) {
+        double a2[3][3], A3[27], A4[81], A5[243], A6[729];
+        for (int m = 0; m < 6; m++) a2[AB[m][0]][AB[m][1]] = a2[AB[m][1]][AB[m][0]] = a1[m];
+        a1_recursion(a2, u, A3, A4, A5, A6);
+        for (int k = 10; k < Q; k++) M[k] += (1.0 - omega_g) * a1_of_mode(k, a2, A3, A4, A5, A6);
+    }
     /* body force, Guo in moment form (R13) */
     for (int a = 0; a < 3; a++) M[1 + a] += 0.5 * F[a];
     for (int m = 0; m < 6; m++) {
@@ -402,7 +464,7 @@ static void collide(const rflbm_ref_t *h, const double g[Q], uint32_t site, uint
         draw_site(h->seed, t, site, h->precision, words, r);
         double sq = sqrt(rho);
         for (int k = 4; k < Q; k++) {
-            double om = (k <= 9) ? omega_h : 1.0;
+            double om = (k <= 9) ? omega_h : omega_g;
             double sigma = sqrt(h->kT * om * (2.0 - om) * T_b[k] / cs2);
             M[k] += sq * sigma * r[k];
         }
@@ -470,6 +532,18 @@ int rflbm_ref_collide_site(const double g[Q], double tau, double kT, uint64_t se
     memset(&h, 0, sizeof(h));
     h.tau = tau; h.kT = kT; h.seed = seed; h.precision = precision;
     if (gacc) { h.g[0] = gacc[0]; h.g[1] = gacc[1]; h.g[2] = gacc[2]; }
+    collide(&h, g, site, t, fstar);
+    return REF_OK;
+}
+
+/* single-site entry with a ghost relaxation time (omega_g = 1/tau_g) */
+int rflbm_ref_collide_site_ghost(const double g[Q], double tau, double tau_g, double kT, uint64_t seed, int precision,
+                                 uint32_t site, uint64_t t, double fstar[Q])
+{
+    build_tables();
+    rflbm_ref_t h;
+    memset(&h, 0, sizeof(h));
+    h.tau = tau; h.tau_g = tau_g; h.kT = kT; h.seed = seed; h.precision = precision;
     collide(&h, g, site, t, fstar);
     return REF_OK;
 }
