@@ -82,6 +82,12 @@ int rflbm_step(rflbm_t* h, int nsteps);
 enum { RFLBM_SCHEME_AB = 0, RFLBM_SCHEME_AA = 1 };
 int rflbm_set_scheme(rflbm_t* h, int scheme);
 
+/* Ghost relaxation time tau_g = 1/omega_g of Reg-FLBM.  Default 1: the paper's final scheme, in
+ * which the ghost part f^(1,g) drops out.  tau_g != 1 adds (1-omega_g) f^(1,g) with the recursive coefficients of
+ * Eq.21 (:163-166, reading R20) and gives the ghost modes the noise amplitude of Eq.9 at omega_g.  Ignored by the
+ * BGK model.  EINVAL: tau_g <= 0.5 or non-finite, or tau_g != 1 with a body force set. */
+int rflbm_set_ghost_tau(rflbm_t* h, double tau_g);
+
 /* Collision model.  RFLBM_MODEL_REG (default): the regularized fluctuating model, Eq.24, the hot
  * path.  RFLBM_MODEL_BGK: the paper's comparison model BGK-FLBM, Eq.11 (:109-111) with Eq.6 (:85): every
  * non-conserved mode k = 4..26 relaxes at the one rate omega = 1/tau and carries noise of amplitude Eq.9 at that

@@ -31,6 +31,7 @@ SYMBOLS = {
     "rflbm_set_force": (_i32, [_vp, _dbl, _dbl, _dbl]),
     "rflbm_set_kernel_variant": (_i32, [_vp, _i32]),
     "rflbm_set_model": (_i32, [_vp, _i32]),
+    "rflbm_set_ghost_tau": (_i32, [_vp, _dbl]),
     "rflbm_set_scheme": (_i32, [_vp, _i32]),
     "rflbm_init": (_i32, [_vp, _vp, _vp]),
     "rflbm_step": (_i32, [_vp, _i32]),
@@ -125,6 +126,9 @@ class Rflbm:
 
     def set_walls_z(self, on=True):
         self._ck(self.lib.rflbm_set_walls_z(self.h, int(on)))
+
+    def set_ghost_tau(self, tau_g):
+        self._ck(self.lib.rflbm_set_ghost_tau(self.h, float(tau_g)))
 
     def set_model(self, model):
         self._ck(self.lib.rflbm_set_model(self.h, int(model)))

@@ -26,6 +26,7 @@ struct rflbm {
     int precision;
     int walls;
     int model;           // RFLBM_MODEL_REG / RFLBM_MODEL_BGK
+    double tau_g;        // ghost relaxation time 1/omega_g (1 = the paper's final scheme)
     int scheme;          // RFLBM_SCHEME_AB (two buffers) / RFLBM_SCHEME_AA (one buffer, in place)
     int aa_phase;        // AA: 0 = natural layout (next step is the in-place one), 1 = after an in-place step
     double g[3];
@@ -128,6 +129,7 @@ extern "C" int rflbm_create(int nx, int ny, int nz, double tau, double kT, doubl
     if (const char* e = getenv("RFLBM_QPAD")) pad = atoll(e) / 32 * 32;          // development knob (bench sweeps)
     h->QS = (h->N + 31) / 32 * 32 + pad;
     if ((double)h->QS >= 4294967296.0) { delete h; return RFLBM_EINVAL; }
+    h->tau_g = 1.0;
     h->tau = tau; h->kT = kT; h->rho0 = rho0; h->seed = seed; h->precision = precision;
     // one thread per site; a warp covers 32 consecutive x whenever nx >= 32
     int bx = 8;
@@ -202,8 +204,8 @@ extern "C" int rflbm_set_force(rflbm_t* h, double gx, double gy, double gz)
 {
     if (!h) return RFLBM_EINVAL;
     if (!std::isfinite(gx) || !std::isfinite(gy) || !std::isfinite(gz)) return fail(h, RFLBM_EINVAL, "non-finite force");
-    if (h->model == RFLBM_MODEL_BGK && (gx != 0.0 || gy != 0.0 || gz != 0.0))
-        return fail(h, RFLBM_EINVAL, "BGK-FLBM carries no body force");
+    if ((h->model == RFLBM_MODEL_BGK || h->tau_g != 1.0) && (gx != 0.0 || gy != 0.0 || gz != 0.0))
+        return fail(h, RFLBM_EINVAL, "BGK-FLBM and the general ghost rate carry no body force");
     h->g[0] = gx; h->g[1] = gy; h->g[2] = gz;
     h->force = (gx != 0.0 || gy != 0.0 || gz != 0.0);
     return RFLBM_OK;
@@ -227,10 +229,12 @@ static StepParams<real> step_params(const rflbm* h, uint64_t t)
     const double omega = 1.0 / h->tau;
     P.nx = h->nx; P.ny = h->ny; P.nz = h->nz; P.N = h->N; P.QS = h->QS;
     P.half_omc = (real)(0.5 * (1.0 - omega));
+    const double omega_g = 1.0 / h->tau_g;
+    P.omc_g = (real)(1.0 - omega_g);
     // Eq.9 per unit sqrt(rho): sqrt(3 kT omega_k (2 - omega_k)) prod_axis s_p, s = (1, sqrt3/6, sqrt2/6)
     // omega_k = omega_h for k = 4..9; ghosts: 1 in Reg-FLBM (:215), the same omega in BGK-FLBM (Eq.11)
     const double nh = std::sqrt(3.0 * h->kT * omega * (2.0 - omega));
-    const double ng = (h->model == RFLBM_MODEL_BGK) ? nh : std::sqrt(3.0 * h->kT);
+    const double ng = (h->model == RFLBM_MODEL_BGK) ? nh : std::sqrt(3.0 * h->kT * omega_g * (2.0 - omega_g));
     const double s1 = std::sqrt(3.0) / 6.0, s2 = std::sqrt(2.0) / 6.0;
     P.amp[AMP_200] = (real)(nh * s2);
     P.amp[AMP_110] = (real)(nh * s1 * s1);
@@ -336,7 +340,7 @@ extern "C" int rflbm_get_populations(rflbm_t* h, void* f_dev)
 }
 
 // ---------------------------------------------------------------- the time step
-template <typename real, bool WALLS, bool FORCE, bool NOISE, bool BGK, int PHASE>
+template <typename real, bool WALLS, bool FORCE, bool NOISE, bool BGK, bool GHOST, int PHASE>
 static void launch_one(rflbm* h, const StepParams<real>& P, bool tma)
 {
     // A-B: read buf[cur], write the other buffer; AA: one buffer, in place
@@ -344,32 +348,37 @@ static void launch_one(rflbm* h, const StepParams<real>& P, bool tma)
     real* dst = (real*)h->buf[PHASE == STEP_AB ? (h->cur ^ 1) : h->cur];
     if (tma) {
         const dim3 grid((h->nx + TILE_X - 1) / TILE_X, (h->ny + h->tma_rows - 1) / h->tma_rows, h->nz);
-        step_kernel_tma<real, WALLS, FORCE, NOISE, BGK, PHASE><<<grid, TILE_X, 0, h->stream>>>(
+        step_kernel_tma<real, WALLS, FORCE, NOISE, BGK, GHOST, PHASE><<<grid, TILE_X, 0, h->stream>>>(
             h->tmap[h->cur], src, dst, P, h->tma_rows);
     } else {
-        step_kernel<real, WALLS, FORCE, NOISE, BGK, PHASE><<<h->grid, h->block, 0, h->stream>>>(src, dst, P);
+        step_kernel<real, WALLS, FORCE, NOISE, BGK, GHOST, PHASE><<<h->grid, h->block, 0, h->stream>>>(src, dst, P);
     }
 }
 
 static bool use_tma(const rflbm* h) { return h->tma_ok && h->variant != RFLBM_KERNEL_PLAIN; }
 
-// variant bits: 8 = BGK-FLBM, 4 = walls, 2 = force, 1 = noise (BGK carries no force: rflbm_set_model / set_force)
+// variant bits: 16 = general ghost rate, 8 = BGK-FLBM, 4 = walls, 2 = force, 1 = noise
+// (BGK and the ghost rate carry no force and exclude each other: rflbm_set_model / set_ghost_tau / set_force)
 template <typename real, int PHASE>
 static void dispatch_variant(rflbm* h, const StepParams<real>& P, int variant, bool tma)
 {
     switch (variant) {
-        case 0: launch_one<real, false, false, false, false, PHASE>(h, P, tma); break;
-        case 1: launch_one<real, false, false, true, false, PHASE>(h, P, tma); break;
-        case 2: launch_one<real, false, true, false, false, PHASE>(h, P, tma); break;
-        case 3: launch_one<real, false, true, true, false, PHASE>(h, P, tma); break;
-        case 4: launch_one<real, true, false, false, false, PHASE>(h, P, tma); break;
-        case 5: launch_one<real, true, false, true, false, PHASE>(h, P, tma); break;
-        case 6: launch_one<real, true, true, false, false, PHASE>(h, P, tma); break;
-        case 7: launch_one<real, true, true, true, false, PHASE>(h, P, tma); break;
-        case 8: launch_one<real, false, false, false, true, PHASE>(h, P, tma); break;
-        case 9: launch_one<real, false, false, true, true, PHASE>(h, P, tma); break;
-        case 12: launch_one<real, true, false, false, true, PHASE>(h, P, tma); break;
-        default: launch_one<real, true, false, true, true, PHASE>(h, P, tma); break;     // 13
+        case 0: launch_one<real, false, false, false, false, false, PHASE>(h, P, tma); break;
+        case 1: launch_one<real, false, false, true, false, false, PHASE>(h, P, tma); break;
+        case 2: launch_one<real, false, true, false, false, false, PHASE>(h, P, tma); break;
+        case 3: launch_one<real, false, true, true, false, false, PHASE>(h, P, tma); break;
+        case 4: launch_one<real, true, false, false, false, false, PHASE>(h, P, tma); break;
+        case 5: launch_one<real, true, false, true, false, false, PHASE>(h, P, tma); break;
+        case 6: launch_one<real, true, true, false, false, false, PHASE>(h, P, tma); break;
+        case 7: launch_one<real, true, true, true, false, false, PHASE>(h, P, tma); break;
+        case 8: launch_one<real, false, false, false, true, false, PHASE>(h, P, tma); break;
+        case 9: launch_one<real, false, false, true, true, false, PHASE>(h, P, tma); break;
+        case 12: launch_one<real, true, false, false, true, false, PHASE>(h, P, tma); break;
+        case 13: launch_one<real, true, false, true, true, false, PHASE>(h, P, tma); break;
+        case 16: launch_one<real, false, false, false, false, true, PHASE>(h, P, tma); break;
+        case 17: launch_one<real, false, false, true, false, true, PHASE>(h, P, tma); break;
+        case 20: launch_one<real, true, false, false, false, true, PHASE>(h, P, tma); break;
+        default: launch_one<real, true, false, true, false, true, PHASE>(h, P, tma); break;    // 21
     }
 }
 
@@ -388,7 +397,8 @@ static int do_step(rflbm* h, int nsteps)
     if (h->variant == RFLBM_KERNEL_TMA && !h->tma_ok)
         return fail(h, RFLBM_EINVAL, "TMA kernel needs nx >= 128 and a row pitch that is a multiple of 16 bytes");
     const bool tma = use_tma(h);
-    const int variant = (h->model == RFLBM_MODEL_BGK ? 8 : 0) | (h->walls ? 4 : 0) | (h->force ? 2 : 0) | (noise ? 1 : 0);
+    const bool ghost = h->model == RFLBM_MODEL_REG && h->tau_g != 1.0;
+    const int variant = (ghost ? 16 : 0) | (h->model == RFLBM_MODEL_BGK ? 8 : 0) | (h->walls ? 4 : 0) | (h->force ? 2 : 0) | (noise ? 1 : 0);
     for (int s = 0; s < nsteps; ++s) {
         const StepParams<real> P = step_params<real>(h, h->t);
         dispatch_step<real>(h, P, variant, tma);
@@ -543,6 +553,15 @@ extern "C" int rflbm_set_scheme(rflbm_t* h, int scheme)
     if (scheme != RFLBM_SCHEME_AB && scheme != RFLBM_SCHEME_AA) return fail(h, RFLBM_EINVAL, "unknown scheme %d", scheme);
     if (h->ws) return fail(h, RFLBM_ESTATE, "rflbm_set_scheme must precede rflbm_set_workspace (the workspace size depends on it)");
     h->scheme = scheme;
+    return RFLBM_OK;
+}
+
+extern "C" int rflbm_set_ghost_tau(rflbm_t* h, double tau_g)
+{
+    if (!h) return RFLBM_EINVAL;
+    if (!std::isfinite(tau_g) || !(tau_g > 0.5)) return fail(h, RFLBM_EINVAL, "tau_g must be finite and > 0.5");
+    if (tau_g != 1.0 && h->force) return fail(h, RFLBM_EINVAL, "the general ghost rate carries no body force");
+    h->tau_g = tau_g;
     return RFLBM_OK;
 }
 

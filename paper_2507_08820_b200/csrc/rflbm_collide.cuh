@@ -41,6 +41,7 @@ struct StepParams {
     long long N;
     long long QS;           // elements between consecutive population arrays (N + padding, see rflbm.cu)
     real half_omc;          // (1 - omega_h)/2
+    real omc_g;             // 1 - omega_g (0 in the paper's final scheme, :215)
     real amp[AMP_N];        // noise amplitude per class (times sqrt(rho) at the site), Eq.9
     real gx, gy, gz;        // acceleration (R13)
     real force_stress;      // 1 - omega_h/2
@@ -150,11 +151,31 @@ __device__ __forceinline__ void back1d(real m0, real m1s, real m2s, real& fm, re
 // BGK = false: Reg-FLBM, Eq.24 (the hot path).  BGK = true: BGK-FLBM, Eq.11 (:109-111), the paper's comparison
 // model: every non-conserved mode relaxes at the one rate omega, M_k = M_k^eq + (1-omega)(m_k - M_k^eq), which
 // needs all 27 moments of the incoming populations (no body force in this model).
-template <typename real, bool FORCE, bool NOISE, bool BGK = false>
+// a1 of ghost mode (p,q,r), order >= 3: the fixed point of the recursion Eq.21 (:163-166, R20) is the sum over index
+// pairs of a1^(2)[pair] times the velocities of the remaining indices.  p, q, r are compile-time after unrolling.
+template <typename real>
+__device__ __forceinline__ real upow(real u, real u2, int n) { return n == 0 ? real(1) : n == 1 ? u : u2; }
+
+template <typename real>
+__device__ __forceinline__ real a1_ghost(int p, int q, int r, const real (&a)[6], const real (&u)[3], const real (&u2)[3])
+{
+    real t = real(0);
+    if (p == 2) t = fma(a[0], upow(u[1], u2[1], q) * upow(u[2], u2[2], r), t);
+    if (q == 2) t = fma(a[1], upow(u[0], u2[0], p) * upow(u[2], u2[2], r), t);
+    if (r == 2) t = fma(a[2], upow(u[0], u2[0], p) * upow(u[1], u2[1], q), t);
+    if (p && q) t = fma(real(p * q) * a[3], upow(u[0], u2[0], p - 1) * upow(u[1], u2[1], q - 1) * upow(u[2], u2[2], r), t);
+    if (p && r) t = fma(real(p * r) * a[4], upow(u[0], u2[0], p - 1) * upow(u[2], u2[2], r - 1) * upow(u[1], u2[1], q), t);
+    if (q && r) t = fma(real(q * r) * a[5], upow(u[1], u2[1], q - 1) * upow(u[2], u2[2], r - 1) * upow(u[0], u2[0], p), t);
+    return t;
+}
+
+// GHOST = true: general ghost rate omega_g != 1 (:211-215): adds (1-omega_g) f^(1,g) with the coefficients of Eq.21.
+template <typename real, bool FORCE, bool NOISE, bool BGK = false, bool GHOST = false>
 __device__ __forceinline__ void collide(real (&g)[3][3][3], const StepParams<real>& P, uint32_t site,
                                         const f64x2* lg, const f64x2* sc)
 {
     static_assert(!(BGK && FORCE), "BGK-FLBM carries no body force");
+    static_assert(!(GHOST && (BGK || FORCE)), "the general ghost rate is built for Reg-FLBM without body force");
     Moments10<real> m;
     real mall[3][3][3];
     if (BGK) {
@@ -213,6 +234,23 @@ __device__ __forceinline__ void collide(real (&g)[3][3][3], const StepParams<rea
         const real dxx = fma(real(-2.0), Ms[2][0][0], fma(real(-1.0 / 3.0), m.rho, m.pxx));
         const real dyy = fma(real(-2.0), Ms[0][2][0], fma(real(-1.0 / 3.0), m.rho, m.pyy));
         const real dzz = fma(real(-2.0), Ms[0][0][2], fma(real(-1.0 / 3.0), m.rho, m.pzz));
+        if (GHOST) {
+            // Eq.21 needs the UNRELAXED a_1^(2) = (dxx, dyy, dzz, axy, axz, ayz) and the equilibrium modes as they are now
+            const real a[6] = {dxx, dyy, dzz, fma(real(-4.0), Ms[1][1][0], m.pxy), fma(real(-4.0), Ms[1][0][1], m.pxz),
+                               fma(real(-4.0), Ms[0][1][1], m.pyz)};
+            const real uu[3] = {ux, uy, uz}, uu2[3] = {ux * ux, uy * uy, uz * uz};
+#pragma unroll
+            for (int p = 0; p < 3; ++p)
+#pragma unroll
+                for (int q = 0; q < 3; ++q)
+#pragma unroll
+                    for (int r = 0; r < 3; ++r) {
+                        if (p + q + r < 3) continue;
+                        const int nnz = (p > 0) + (q > 0) + (r > 0);
+                        const real w = P.omc_g * (nnz == 1 ? real(0.5) : nnz == 2 ? real(0.25) : real(0.125));
+                        Ms[p][q][r] = fma(w, a1_ghost<real>(p, q, r, a, uu, uu2), Ms[p][q][r]);
+                    }
+        }
         Ms[2][0][0] = fma(k2, dxx, Ms[2][0][0]);
         Ms[0][2][0] = fma(k2, dyy, Ms[0][2][0]);
         Ms[0][0][2] = fma(k2, dzz, Ms[0][0][2]);

@@ -121,7 +121,7 @@ __device__ __forceinline__ void scatter(real* dst, long long QS, int nx, int ny,
     }
 }
 
-template <typename real, bool WALLS, bool FORCE, bool NOISE, bool BGK, int PHASE>
+template <typename real, bool WALLS, bool FORCE, bool NOISE, bool BGK, bool GHOST, int PHASE>
 __global__ void __launch_bounds__(128)
 step_kernel(const real* src, real* dst, const __grid_constant__ StepParams<real> P)
 {
@@ -134,7 +134,7 @@ step_kernel(const real* src, real* dst, const __grid_constant__ StepParams<real>
     real g[3][3][3];
     gather<real, WALLS, PHASE == STEP_AB ? GATHER_AB : PHASE == STEP_AA_EVEN ? GATHER_AA0 : GATHER_AA1>(
         src, P.QS, P.nx, P.ny, P.nz, i, g);
-    collide<real, FORCE, NOISE, BGK>(g, P, (uint32_t)i.s, s_tab, s_tab + LOG_TABLE_N);
+    collide<real, FORCE, NOISE, BGK, GHOST>(g, P, (uint32_t)i.s, s_tab, s_tab + LOG_TABLE_N);
     scatter<real, WALLS, PHASE>(dst, P.QS, P.nx, P.ny, P.nz, i, g);
 }
 

@@ -116,7 +116,7 @@ __device__ __forceinline__ void issue_tile(const CUtensorMap* tmap, uint32_t s_i
 }
 
 // fp64: 128 registers, 41 KB -> 4 blocks per SM; fp32: 64 registers, 15 KB -> 8 blocks per SM
-template <typename real, bool WALLS, bool FORCE, bool NOISE, bool BGK, int PHASE>
+template <typename real, bool WALLS, bool FORCE, bool NOISE, bool BGK, bool GHOST, int PHASE>
 __global__ void __launch_bounds__(TILE_X, sizeof(real) == 8 ? 4 : 8)
 step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const real* src, real* dst,
                 const __grid_constant__ StepParams<real> P, int rows)
@@ -225,7 +225,7 @@ step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const real* src, r
             }
         }
         if (active) {
-            collide<real, FORCE, NOISE, BGK>(g, P, (uint32_t)s, s_tab, s_tab + LOG_TABLE_N);
+            collide<real, FORCE, NOISE, BGK, GHOST>(g, P, (uint32_t)s, s_tab, s_tab + LOG_TABLE_N);
             if (PHASE == STEP_AA_ODD) {
                 // push to the neighbours x + c_q (slot q), misaligned by one element for cx = +-1: the partial
                 // sectors at the ends of a warp's 256 bytes are completed in L2 by the neighbouring warp's store

@@ -369,3 +369,29 @@ def test_aa_set_get_roundtrip_resume_and_bgk():
     a = binding.Rflbm(20, 8, 6, 0.7, 1e-4, 1.0, 3, scheme=binding.SCHEME_AA); a.set_model(binding.MODEL_BGK); a.init(); a.step(15)
     b = binding.Rflbm(20, 8, 6, 0.7, 1e-4, 1.0, 3); b.set_model(binding.MODEL_BGK); b.init(); b.step(15)
     assert torch.equal(a.get_populations(), b.get_populations())
+
+
+@pytest.mark.parametrize("shape,prec,walls,kT,tau,tau_g,scheme", [
+    ((16, 16, 16), binding.F64, False, 1e-4, 0.8, 1.6, binding.SCHEME_AB), ((5, 7, 9), binding.F64, True, 1e-4, 0.55, 0.7, binding.SCHEME_AA),
+    ((132, 6, 5), binding.F64, True, 1e-4, 3.0, 0.6, binding.SCHEME_AB), ((256, 4, 3), binding.F64, False, 0.0, 0.9, 2.5, binding.SCHEME_AA),
+    ((136, 5, 6), binding.F32, False, 1e-4, 0.8, 1.3, binding.SCHEME_AB)])
+def test_general_ghost_rate_matches_oracle(shape, prec, walls, kT, tau, tau_g, scheme):
+    """omega_g != 1 (Eq.21 live): GPU closed-form pair sums against the oracle's literal tensor recursion."""
+    torch = torch_()
+    nx, ny, nz = shape
+    fields = synthetic.smooth_random_fields(nx, ny, nz, 41)
+    sim = binding.Rflbm(nx, ny, nz, tau, kT, 1.0, 43, prec, scheme=scheme)
+    ref = oracle.Ref(nx, ny, nz, tau, kT, 1.0, 43, prec, threads=NT)
+    if walls:
+        sim.set_walls_z(True); ref.set_walls_z(True)
+    sim.set_ghost_tau(tau_g); ref.set_ghost_tau(tau_g)
+    init_pair(sim, ref, fields)
+    sim.step(61); ref.step(61)
+    err = np.abs(pops(sim) - ref.get_populations()).max()
+    assert err < (TOL64 if prec == binding.F64 else TOL32), err
+    with pytest.raises(binding.RflbmError):
+        sim.set_force(1e-6, 0.0, 0.0)
+    # tau_g = 1 is the default path bit for bit
+    a = binding.Rflbm(12, 6, 5, 0.8, 1e-4, 1.0, 3); a.set_ghost_tau(1.0); a.init(); a.step(9)
+    b = binding.Rflbm(12, 6, 5, 0.8, 1e-4, 1.0, 3); b.init(); b.step(9)
+    assert torch.equal(a.get_populations(), b.get_populations())
