@@ -290,7 +290,9 @@ def run_ours(args):
     achieved = bytes_per_launch / (ms_local / K * 1e-3) / 1e9
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": ncu_traffic_bytes(n, args.precision), "peak_source": peak_src,
-                "kernel": "step_kernel", "algorithmic_bytes_per_launch": bytes_per_launch,
+                "kernel": ("step_kernel_tma" if (args.variant != "plain" and n >= 128 and n % (16 // es) == 0
+                                                 and (args.kT > 0 or args.variant == "tma")) else "step_kernel"),
+                "algorithmic_bytes_per_launch": bytes_per_launch,
                 "avg_launch_ms": ms_local / K}
 
     cpu = None

@@ -97,8 +97,8 @@ int rflbm_set_ghost_tau(rflbm_t* h, double tau_g);
 enum { RFLBM_MODEL_REG = 0, RFLBM_MODEL_BGK = 1 };
 int rflbm_set_model(rflbm_t* h, int model);
 
-/* Which implementation of the step kernel rflbm_step launches.  AUTO (default): the TMA-staged kernel when the
- * lattice allows it (nx >= 128 and nx*sizeof(real) a multiple of 16), else the plain one-thread-per-site kernel.  PLAIN forces the
+/* Which implementation of the step kernel rflbm_step launches.  AUTO (default): the TMA-staged kernel when kT > 0
+ * and the lattice allows it (nx >= 128 and nx*sizeof(real) a multiple of 16), else the plain one-thread-per-site kernel.  PLAIN forces the
  * latter; TMA fails with EINVAL at rflbm_step if the lattice does not allow it.  All variants compute the same
  * update (same results up to the bit: identical arithmetic, only the data movement differs). */
 enum { RFLBM_KERNEL_AUTO = 0, RFLBM_KERNEL_PLAIN = 1, RFLBM_KERNEL_TMA = 2 };
