@@ -207,3 +207,43 @@ def test_table_III_trend_equilibration_ratios_64(model, tau):
     # tau = 0.51 sits at the edge of the paper's 0.5 % band: Table III prints 1.005 / 1.013 / 1.004 / 1.012 there
     # (measured here: 1.003 / 1.006 / 1.006 / 1.005)
     assert np.abs(er - 1.0).max() < (0.015 if tau < 0.55 else 0.005), er
+
+
+def test_largest_lattice_768_in_place_sampled_against_oracle():
+    """Maximum size on a 180 GB part: 768^3 fp64 in the AA scheme (97.8 GB in one buffer; site indices up to 4.5e8,
+    byte offsets up to 9.8e10).  After ONE step from the uniform start the state at a site is fully determined by
+    the 27 neighbouring collisions of f = w (each with its own Philox counter), which the oracle evaluates one by one:
+    S_1[q](x) = collide(w; site = x - c_q, t = 0)[q].  rho and u of sampled sites (corners, tile edges, the last
+    site) are compared through rflbm_moments; then a second (odd-phase) step must conserve mass and momentum."""
+    torch = torch_()
+    n, tau, kT, seed = 768, 0.8, 1e-4, 11
+    free, _ = torch.cuda.mem_get_info()
+    if free < 120e9:
+        pytest.skip("needs 120 GB of free device memory")
+    sim = binding.Rflbm(n, n, n, tau, kT, 1.0, seed, scheme=binding.SCHEME_AA)
+    assert sim.workspace.numel() < 99e9
+    sim.init()
+    sim.step(1)
+    rho, u = sim.moments()
+    c, w = oracle.tables()[:2]
+    rng = np.random.default_rng(8)
+    pts = rng.integers(0, n, size=(40, 3)).tolist()
+    pts += [(0, 0, 0), (n - 1, n - 1, n - 1), (0, n - 1, 0), (127, 5, 767), (128, 767, 3), (767, 0, 400), (640, 15, 16)]
+    worst = 0.0
+    for x, y, z in pts:
+        s1 = np.zeros(27)
+        for q in range(27):
+            xs, ys, zs = (x - c[q][0]) % n, (y - c[q][1]) % n, (z - c[q][2]) % n
+            s1[q] = oracle.collide_site(w, tau, kT, seed, site=int(xs + n * (ys + n * zs)), t=0)[q]
+        r = s1.sum()
+        uu = (s1 @ c) / r
+        worst = max(worst, abs(float(rho[z, y, x]) - r), float(np.abs(u[:, z, y, x].cpu().numpy() - uu).max()))
+    assert worst < 1e-14, worst
+    del rho, u
+    d1 = sim.diagnostics()
+    sim.step(1)                                                  # odd phase: pushes to the neighbours
+    d2 = sim.diagnostics()
+    N = n ** 3
+    # sums of 4.5e8 terms through fp64 atomics: rounding of the accumulation itself is ~1e-13 relative
+    assert abs(d1[0] / N - 1.0) < 1e-12 and abs(d2[0] - d1[0]) / N < 1e-12
+    assert max(abs(v) for v in d2[1:4]) / N < 1e-14
