@@ -31,3 +31,19 @@ def shell_spectrum(field, mean_sub=True):
     tot = np.bincount(shell.ravel(), weights=p.ravel(), minlength=nsh)
     cnt = np.bincount(shell.ravel(), minlength=nsh)
     return tot, cnt
+
+
+def shell_spectrum_torch(field, mean_sub=True):
+    """shell_spectrum on the GPU (torch.fft): |FFT|^2 / N binned by round(|k| L / 2 pi); returns numpy (tot, cnt)."""
+    import torch
+    f = field.double()
+    if mean_sub:
+        f = f - f.mean()
+    p = (torch.fft.fftn(f).abs() ** 2 / f.numel()).reshape(-1)
+    axes = [torch.fft.fftfreq(s, 1.0 / s, device=f.device, dtype=torch.float64) for s in f.shape]
+    kk = torch.sqrt(sum(a ** 2 for a in torch.meshgrid(*axes, indexing="ij")))
+    shell = torch.round(kk).long().reshape(-1)
+    nsh = int(shell.max()) + 1
+    tot = torch.bincount(shell, weights=p, minlength=nsh)
+    cnt = torch.bincount(shell, minlength=nsh)
+    return tot.cpu().numpy(), cnt.cpu().numpy()
