@@ -96,6 +96,8 @@ def test_config4_sampled_parity_and_conservation_512():
     single-site collision (exact neighbours through the periodic wrap), then conservation over the run."""
     torch = torch_()
     n, tau, kT, seed = 512, 0.8, 1e-4, 11
+    import gc
+    gc.collect(); torch.cuda.empty_cache()                     # earlier tests' cached blocks do not count as free
     free, _ = torch.cuda.mem_get_info()
     if free < 125e9:
         pytest.skip("needs 125 GB of free device memory")
@@ -217,6 +219,8 @@ def test_largest_lattice_768_in_place_sampled_against_oracle():
     site) are compared through rflbm_moments; then a second (odd-phase) step must conserve mass and momentum."""
     torch = torch_()
     n, tau, kT, seed = 768, 0.8, 1e-4, 11
+    import gc
+    gc.collect(); torch.cuda.empty_cache()
     free, _ = torch.cuda.mem_get_info()
     if free < 120e9:
         pytest.skip("needs 120 GB of free device memory")
