@@ -26,9 +26,9 @@ struct rflbm {
     bool force;
     void* ws;            // borrowed workspace
     size_t ws_bytes;
-    void* buf[2];        // A-B population buffers inside ws
+    void* buf[2];        // population buffers inside ws (AA: buf[1] is NULL)
     double* acc;         // 4 KiB reduction scratch inside ws
-    f64x2* tables;       // 8 KiB Box-Muller tables inside ws (uploaded by set_workspace)
+    f64x2* tables;       // 12 KiB Box-Muller tables inside ws (uploaded by set_workspace)
     int cur;             // buffer holding P_{t-1}
     bool inited;
     uint64_t t;

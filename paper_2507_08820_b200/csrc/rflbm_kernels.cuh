@@ -1,10 +1,13 @@
 // rflbm_kernels.cuh — CUDA kernels of the Reg-FLBM path (sm_100a).
 //
-// Storage: two SoA buffers P[q][z][y][x] of `real` in the lex order of
-// rflbm_lattice.cuh, holding POST-collision, UN-streamed populations (R10).  A step PULLS
-// S_t[q](x) = P_{t-1}[q](x - c_q)  (Eq.7 :87; bounce-back: P_{t-1}[26-q](x) when x - c_q is solid, R12),
-// collides in registers and stores P_t[q](x): 27 neighbour reads (coalesced, at most one element off
-// alignment) and 27 aligned coalesced writes per site, nothing else.
+// Storage: SoA buffers P[q][z][y][x] of `real` in the lex order of rflbm_lattice.cuh, the 27
+// arrays QS elements apart.
+//   A-B scheme: two buffers holding POST-collision, UN-streamed populations (R10).  A step PULLS
+//     S_t[q](x) = P_{t-1}[q](x - c_q)  (Eq.7 :87; bounce-back: P_{t-1}[26-q](x) when x - c_q is solid, R12),
+//     collides in registers and stores P_t[q](x): 27 neighbour reads (coalesced, at most one element off alignment)
+//     and 27 aligned coalesced writes per site, nothing else.
+//   AA scheme: one buffer updated in place, alternating an all-local step and a pull/push step (STEP_AA_EVEN/ODD).
+// The observables gather the pre-collision state S_t according to scheme and phase (GATHER_*).
 #pragma once
 #include "rflbm_collide.cuh"
 
@@ -70,7 +73,7 @@ __device__ __forceinline__ void gather(const real* __restrict__ src, long long Q
     }
 }
 
-// copy the Box-Muller tables (8 KB) from global memory (L2 resident) to shared memory; ends with a barrier
+// copy the Box-Muller tables (12 KB) from global memory (L2 resident) to shared memory; ends with a barrier
 __device__ __forceinline__ void stage_tables(const f64x2* __restrict__ tab, f64x2* s_tab)
 {
     const int tid = threadIdx.y * blockDim.x + threadIdx.x, nt = blockDim.x * blockDim.y;
