@@ -137,7 +137,7 @@ extern "C" int rflbm_set_workspace(rflbm_t* h, void* dev_ptr, size_t bytes)
     if (int rc0 = check_cuda(h, cudaMemset(h->acc, 0, 4096), "scratch clear")) return rc0;
     // the only device writes outside the stream: the scratch clear above and the Box-Muller tables
     // (host-generated, long double libm)
-    static f64x2 host_tab[LOG_TABLE_N + SC_TABLE_N];
+    f64x2 host_tab[LOG_TABLE_N + SC_TABLE_N];                  // 12 KB on the stack: no shared state between handles
     fill_normal_tables(host_tab, host_tab + LOG_TABLE_N);
     const int rc = check_cuda(h, cudaMemcpy(h->tables, host_tab, TABLE_BYTES, cudaMemcpyHostToDevice), "table upload");
     if (rc != RFLBM_OK) return rc;
