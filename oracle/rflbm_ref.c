@@ -29,7 +29,11 @@
  * Box-Muller closed-form points and sample statistics; mass/momentum conservation;
  * equilibrium fixed point and product closed form; post-collision moment structure;
  * brute-force streaming on tiny boxes; Taylor-Green decay rate nu=(tau-1/2)/3;
- * equipartition of all 27 modes; flat structure factor; Poiseuille profile with walls+force.
+ * equipartition of all 27 modes; flat structure factor; Poiseuille profile with walls+force;
+ * diagnostics mean/variance over fluid sites against the printed basis rows 0..3 and closed forms
+ * (tests/test_oracle_diagnostics.py); the fp32 storage mode: every stored value is a float after init
+ * and after every step in all three store sites, one step = rounded single-site collision streamed by
+ * numpy, 24-bit uniforms (tests/test_oracle_fp32.py).
  * Parity unpinned: near-wall fluctuation variance with walls (nothing fixes it).
  */
 #include <math.h>
