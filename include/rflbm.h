@@ -40,17 +40,20 @@ enum { RFLBM_OK = 0, RFLBM_EINVAL = -1, RFLBM_ESTATE = -2, RFLBM_ENOMEM = -3, RF
  * PAPER.md:52; ghost rate omega_g = 1, :215), thermal energy kT (Eq.9 :99; kT = 0 -> deterministic
  * Reg-LBM, :294), reference density rho0 (:252), Philox seed (R8) and precision.
  * Host only: no GPU work, no allocation on the device.
- * EINVAL: nx,ny,nz < 1, N >= 2^32, tau <= 0.5 or non-finite, kT < 0, rho0 <= 0, unknown precision, out NULL. */
+ * EINVAL: nx,ny,nz < 1, N >= 2^32, ny > 65535 * max(1, 128/nx rounded down to a power of two) or nz > 65535 (launch
+ * grid limits), tau <= 0.5 or non-finite, kT < 0, rho0 <= 0, unknown precision, out NULL. */
 int rflbm_create(int nx, int ny, int nz, double tau, double kT, double rho0, uint64_t seed, int precision,
                  rflbm_t** out);
 
 /* Bytes of device workspace the handle needs: two population buffers 2*27*QS*sizeof(real) (A-B scheme; one for AA;
- * QS = N rounded up to 32 plus a 9.5 KB skew for N >= 65536)
- * plus a 4 KiB reduction scratch and 12 KiB of Box-Muller tables (uploaded by rflbm_set_workspace, synchronously). */
+ * QS = storage sites px*ny*nzs rounded up to 32 plus a 9.5 KB skew when >= 65536, px = nx rounded up to whole 128-byte
+ * lines for nx >= 32, nzs = nz, or nz+2 in slab mode) plus a 4 KiB reduction scratch and 12 KiB of Box-Muller tables. */
 size_t rflbm_workspace_bytes(const rflbm_t* h);
 
 /* Borrow `bytes` of device memory at dev_ptr (256-byte aligned) as the workspace.
- * ENOMEM if too small or misaligned.  Invalidates the state (rflbm_init / rflbm_set_populations needed). */
+ * ENOMEM if too small or misaligned.  Invalidates the state (rflbm_init / rflbm_set_populations needed).
+ * The one call that writes to the device outside the handle's stream: it clears the 4 KiB scratch and uploads the
+ * Box-Muller tables on the legacy stream and waits for both before returning (host-synchronous). */
 int rflbm_set_workspace(rflbm_t* h, void* dev_ptr, size_t bytes);
 
 /* cudaStream_t (as void*) on which every later call enqueues its work; borrowed. */
@@ -82,6 +85,40 @@ int rflbm_step(rflbm_t* h, int nsteps);
 enum { RFLBM_SCHEME_AB = 0, RFLBM_SCHEME_AA = 1 };
 int rflbm_set_scheme(rflbm_t* h, int scheme);
 
+/* z-slab decomposition (PAPER.md:292 "the system was extended along the z direction", :300 "linear decomposition"):
+ * this handle owns the nz layers [z0, z0+nz) of a GLOBAL lattice nx x ny x nz_global, periodic in z over nz_global.
+ * The solid-layer test (walls at global z = 0 and nz_global-1) and the Philox site key x + nx (y + ny z) (R8) use the
+ * global z, so the slabs together compute, bit for bit, what one handle of the undivided lattice computes.
+ * The internal buffers get one ghost layer below and above; the faces travel through the four halo calls below,
+ * which the CALLER moves between handles (cudaMemcpyAsync device-to-device, peer copy, NCCL/MPI send-recv ...): the
+ * library itself never communicates.  In slab mode
+ *   - the fields given to rflbm_init / rflbm_set_populations carry nz+2 layers: global layers z0-1 .. z0+nz
+ *     (periodic in nz_global), i.e. rho[(nz+2)*ny*nx], u[3][...], f[27][...]; outputs have nz layers;
+ *   - rflbm_step advances ONE step per call and, like the observables, fails with ESTATE while an exchange is
+ *     pending (rflbm_halo_pending);
+ *   - rflbm_run_host is not available.
+ * Must be called before rflbm_set_workspace (ESTATE afterwards).  EINVAL: slab outside [0, nz_global), global lattice
+ * with 2^32 sites or more, walls with nz_global < 3. */
+int rflbm_set_slab(rflbm_t* h, int z0, int nz_global);
+
+/* Face exchange of a slab.  Protocol, after rflbm_init / rflbm_set_populations and after every rflbm_step, with all
+ * slabs at the same step count:
+ *     if (rflbm_halo_pending(h)):   rflbm_halo_pack(h, LOW, a);  rflbm_halo_pack(h, HIGH, b);
+ *                                   a -> the neighbour BELOW, which calls rflbm_halo_unpack(., HIGH, a)
+ *                                   b -> the neighbour ABOVE, which calls rflbm_halo_unpack(., LOW,  b)
+ * (periodic: the lowest slab's neighbour below is the highest slab).  A face buffer is 9 populations on one nx x ny
+ * layer, packed [9][ny][nx] of `real`: rflbm_halo_bytes = 9*nx*ny*sizeof(real) (4.7 MB at 256^2 fp64).  What it
+ * carries depends on the storage scheme and phase and is the library's business: the nine c_z = -1 (LOW) / c_z = +1
+ * (HIGH) post-collision populations of the boundary layer that the neighbour will pull (A-B, and AA after an even
+ * step), or, after an odd AA step, the nine populations this slab pushed across the face, which the neighbour takes
+ * home into its own boundary layer.  pack and unpack enqueue one small kernel on the handle's stream and return;
+ * they are no-ops (RFLBM_OK) when nothing is pending.  ESTATE: not in slab mode, or before init. */
+enum { RFLBM_SIDE_LOW = 0, RFLBM_SIDE_HIGH = 1 };
+size_t rflbm_halo_bytes(const rflbm_t* h);
+int rflbm_halo_pending(const rflbm_t* h);
+int rflbm_halo_pack(rflbm_t* h, int side, void* face_dev);
+int rflbm_halo_unpack(rflbm_t* h, int side, const void* face_dev);
+
 /* Ghost relaxation time tau_g = 1/omega_g of Reg-FLBM.  Default 1: the paper's final scheme, in
  * which the ghost part f^(1,g) drops out.  tau_g != 1 adds (1-omega_g) f^(1,g) with the recursive coefficients of
  * Eq.21 (:163-166, reading R20) and gives the ghost modes the noise amplitude of Eq.9 at omega_g.  Ignored by the
@@ -98,8 +135,8 @@ enum { RFLBM_MODEL_REG = 0, RFLBM_MODEL_BGK = 1 };
 int rflbm_set_model(rflbm_t* h, int model);
 
 /* Which implementation of the step kernel rflbm_step launches.  AUTO (default): the TMA-staged kernel when kT > 0
- * and the lattice allows it (nx >= 128 and nx*sizeof(real) a multiple of 16), else the plain one-thread-per-site kernel.  PLAIN forces the
- * latter; TMA fails with EINVAL at rflbm_step if the lattice does not allow it.  All variants compute the same
+ * and nx >= 32 (tiles of 128, 64 or 32 sites; the internal row pitch is padded so that any such nx qualifies), else
+ * the plain one-thread-per-site kernel.  PLAIN forces the latter; TMA fails with EINVAL at rflbm_step if nx < 32.  All variants compute the same
  * update (same results up to the bit: identical arithmetic, only the data movement differs). */
 enum { RFLBM_KERNEL_AUTO = 0, RFLBM_KERNEL_PLAIN = 1, RFLBM_KERNEL_TMA = 2 };
 int rflbm_set_kernel_variant(rflbm_t* h, int variant);
@@ -136,6 +173,10 @@ int rflbm_run_host(rflbm_t* h, const void* rho_host, const void* u_host, int nst
 
 /* Number of kernels the handle has launched so far (bench.py's gpu_launches). */
 uint64_t rflbm_launch_count(const rflbm_t* h);
+
+/* Name of the step kernel the last rflbm_step launched ("step_kernel", "step_kernel_tma<TX=128>", ...; "" before the
+ * first step): a static string, what bench.py reports as roofline.kernel. */
+const char* rflbm_last_kernel(const rflbm_t* h);
 
 uint64_t rflbm_step_count(const rflbm_t* h);
 const char* rflbm_last_error(const rflbm_t* h);

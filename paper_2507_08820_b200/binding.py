@@ -14,10 +14,11 @@ OK, EINVAL, ESTATE, ENOMEM, ECUDA = 0, -1, -2, -3, -4
 KERNEL_AUTO, KERNEL_PLAIN, KERNEL_TMA = 0, 1, 2
 MODEL_REG, MODEL_BGK = 0, 1
 SCHEME_AB, SCHEME_AA = 0, 1
+SIDE_LOW, SIDE_HIGH = 0, 1
 Q = 27
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.environ.get("RFLBM_LIB") or os.path.join(_HERE, "csrc", "librflbm.so")   # env: development builds
+LIB_PATH = os.path.join(_HERE, "csrc", "librflbm.so")
 _lib = None
 
 # every symbol include/rflbm.h declares: name -> (restype, argtypes)
@@ -33,6 +34,11 @@ SYMBOLS = {
     "rflbm_set_model": (_i32, [_vp, _i32]),
     "rflbm_set_ghost_tau": (_i32, [_vp, _dbl]),
     "rflbm_set_scheme": (_i32, [_vp, _i32]),
+    "rflbm_set_slab": (_i32, [_vp, _i32, _i32]),
+    "rflbm_halo_bytes": (_sz, [_vp]),
+    "rflbm_halo_pending": (_i32, [_vp]),
+    "rflbm_halo_pack": (_i32, [_vp, _i32, _vp]),
+    "rflbm_halo_unpack": (_i32, [_vp, _i32, _vp]),
     "rflbm_init": (_i32, [_vp, _vp, _vp]),
     "rflbm_step": (_i32, [_vp, _i32]),
     "rflbm_moments": (_i32, [_vp, _vp, _vp]),
@@ -43,6 +49,7 @@ SYMBOLS = {
     "rflbm_debug_rng": (_i32, [_vp, _u64, _vp, _vp]),
     "rflbm_run_host": (_i32, [_vp, _vp, _vp, _i32, _vp, _vp, _vp, _sz]),
     "rflbm_launch_count": (_u64, [_vp]),
+    "rflbm_last_kernel": (C.c_char_p, [_vp]),
     "rflbm_step_count": (_u64, [_vp]),
     "rflbm_last_error": (C.c_char_p, [_vp]),
     "rflbm_destroy": (_i32, [_vp]),
@@ -78,10 +85,18 @@ def _ptr(t):
 
 class Rflbm:
     """One simulation handle.  Tensors are torch CUDA tensors in the x-fastest layout
-    rho[nz,ny,nx], u[3,nz,ny,nx], f[27,nz,ny,nx] (canonical velocity order), dtype float64 or float32."""
+    rho[nz,ny,nx], u[3,nz,ny,nx], f[27,nz,ny,nx] (canonical velocity order), dtype float64 or float32.
+
+    Stream / device contract: every method runs under `torch.cuda.device(self.device)` and
+    `torch.cuda.stream(self.stream)` (the stream given at construction, default: the stream current at construction),
+    so the tensors it converts or allocates and the kernels the library enqueues are ordered on that one stream.
+    A caller that consumes the returned tensors on another stream must order against `self.stream` itself.
+
+    slab=(z0, nz_global): this handle owns layers [z0, z0+nz) of a global lattice (include/rflbm.h, rflbm_set_slab);
+    init / set_populations then take fields with nz+2 layers and the halo_* methods move the faces."""
 
     def __init__(self, nx, ny, nz, tau, kT, rho0=1.0, seed=0, precision=F64, device="cuda:0", stream=None,
-                 scheme=SCHEME_AB):
+                 scheme=SCHEME_AB, slab=None):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("CUDA is not available: the rflbm path has no CPU fallback")
@@ -89,6 +104,7 @@ class Rflbm:
         self.lib = load()
         self.nx, self.ny, self.nz = nx, ny, nz
         self.shape = (nz, ny, nx)
+        self.shape_in = (nz + 2, ny, nx) if slab is not None else self.shape
         self.n = nx * ny * nz
         self.precision = precision
         self.dtype = torch.float64 if precision == F64 else torch.float32
@@ -100,17 +116,26 @@ class Rflbm:
         self.h = h
         if scheme != SCHEME_AB:
             self._ck(self.lib.rflbm_set_scheme(self.h, int(scheme)))
+        if slab is not None:
+            self._ck(self.lib.rflbm_set_slab(self.h, int(slab[0]), int(slab[1])))
         nbytes = self.lib.rflbm_workspace_bytes(self.h)
         with torch.cuda.device(self.device):
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
             self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)   # owned here, borrowed by C
             self._ck(self.lib.rflbm_set_workspace(self.h, self.workspace.data_ptr(), nbytes))
-            st = stream if stream is not None else torch.cuda.current_stream(self.device)
-            self.stream = st
-            self._ck(self.lib.rflbm_set_stream(self.h, st.cuda_stream))
+            self._ck(self.lib.rflbm_set_stream(self.h, self.stream.cuda_stream))
 
     def _ck(self, rc):
         if rc != OK:
             raise RflbmError(rc, self.lib.rflbm_last_error(self.h).decode())
+
+    def _ctx(self):
+        """device + stream of the handle for the duration of a call (see the class docstring)"""
+        import contextlib
+        st = contextlib.ExitStack()
+        st.enter_context(self.torch.cuda.device(self.device))
+        st.enter_context(self.torch.cuda.stream(self.stream))
+        return st
 
     def close(self):
         if getattr(self, "h", None):
@@ -139,68 +164,105 @@ class Rflbm:
     def set_force(self, gx, gy, gz):
         self._ck(self.lib.rflbm_set_force(self.h, gx, gy, gz))
 
-    def _field(self, t, lead=()):
+    def _field(self, t, lead=(), shape=None):
         t = t.to(device=self.device, dtype=self.dtype).contiguous()
-        assert tuple(t.shape) == tuple(lead) + self.shape, (t.shape, lead, self.shape)
+        shape = self.shape if shape is None else shape
+        assert tuple(t.shape) == tuple(lead) + tuple(shape), (t.shape, lead, shape)
         return t
 
     def init(self, rho=None, u=None):
-        if rho is None:
-            self._ck(self.lib.rflbm_init(self.h, None, None))
-        else:
-            rho, u = self._field(rho), self._field(u, (3,))
-            self._ck(self.lib.rflbm_init(self.h, rho.data_ptr(), u.data_ptr()))
-            self._keep = (rho, u)     # alive until the stream has consumed them
+        with self._ctx():
+            if rho is None:
+                self._ck(self.lib.rflbm_init(self.h, None, None))
+            else:
+                rho, u = self._field(rho, (), self.shape_in), self._field(u, (3,), self.shape_in)
+                self._ck(self.lib.rflbm_init(self.h, rho.data_ptr(), u.data_ptr()))
+                self._keep = (rho, u)     # alive until the stream has consumed them
 
     def step(self, n=1):
-        self._ck(self.lib.rflbm_step(self.h, int(n)))
+        with self._ctx():
+            self._ck(self.lib.rflbm_step(self.h, int(n)))
 
     def moments(self, rho=None, u=None):
         t = self.torch
-        if rho is None:
-            rho = t.empty(self.shape, dtype=self.dtype, device=self.device)
-            u = t.empty((3,) + self.shape, dtype=self.dtype, device=self.device)
-        self._ck(self.lib.rflbm_moments(self.h, rho.data_ptr(), u.data_ptr()))
+        with self._ctx():
+            if rho is None:
+                rho = t.empty(self.shape, dtype=self.dtype, device=self.device)
+                u = t.empty((3,) + self.shape, dtype=self.dtype, device=self.device)
+            self._ck(self.lib.rflbm_moments(self.h, rho.data_ptr(), u.data_ptr()))
         return rho, u
 
     def stress(self, pi=None):
-        if pi is None:
-            pi = self.torch.empty((6,) + self.shape, dtype=self.dtype, device=self.device)
-        self._ck(self.lib.rflbm_stress(self.h, pi.data_ptr()))
+        with self._ctx():
+            if pi is None:
+                pi = self.torch.empty((6,) + self.shape, dtype=self.dtype, device=self.device)
+            self._ck(self.lib.rflbm_stress(self.h, pi.data_ptr()))
         return pi
 
     def diagnostics(self):
         out = (_dbl * 10)()
-        self._ck(self.lib.rflbm_diagnostics(self.h, out))
+        with self._ctx():
+            self._ck(self.lib.rflbm_diagnostics(self.h, out))
         return list(out)
 
     def get_populations(self, f=None):
-        if f is None:
-            f = self.torch.empty((Q,) + self.shape, dtype=self.dtype, device=self.device)
-        self._ck(self.lib.rflbm_get_populations(self.h, f.data_ptr()))
+        with self._ctx():
+            if f is None:
+                f = self.torch.empty((Q,) + self.shape, dtype=self.dtype, device=self.device)
+            self._ck(self.lib.rflbm_get_populations(self.h, f.data_ptr()))
         return f
 
     def set_populations(self, f, step=0):
-        f = self._field(f, (Q,))
-        self._ck(self.lib.rflbm_set_populations(self.h, f.data_ptr(), int(step)))
-        self._keep = (f,)
+        with self._ctx():
+            f = self._field(f, (Q,), self.shape_in)
+            self._ck(self.lib.rflbm_set_populations(self.h, f.data_ptr(), int(step)))
+            self._keep = (f,)
 
     def debug_rng(self, step):
         t = self.torch
-        words = t.empty((24,) + self.shape, dtype=t.int32, device=self.device)
-        normals = t.empty((23,) + self.shape, dtype=self.dtype, device=self.device)
-        self._ck(self.lib.rflbm_debug_rng(self.h, int(step), words.data_ptr(), normals.data_ptr()))
+        with self._ctx():
+            words = t.empty((24,) + self.shape, dtype=t.int32, device=self.device)
+            normals = t.empty((23,) + self.shape, dtype=self.dtype, device=self.device)
+            self._ck(self.lib.rflbm_debug_rng(self.h, int(step), words.data_ptr(), normals.data_ptr()))
         return words, normals
 
     def run_host(self, rho_host, u_host, nsteps, rho_out_host, u_out_host, scratch=None):
         """End-to-end job on HOST tensors (pinned for speed): upload, init, step, moments, download, sync."""
         t = self.torch
         es = 8 if self.precision == F64 else 4
-        if scratch is None:
-            scratch = t.empty(4 * self.n * es, dtype=t.uint8, device=self.device)
-        self._ck(self.lib.rflbm_run_host(self.h, _ptr(rho_host), _ptr(u_host), int(nsteps), rho_out_host.data_ptr(),
-                                         u_out_host.data_ptr(), scratch.data_ptr(), scratch.numel()))
+        with self._ctx():
+            if scratch is None:
+                scratch = t.empty(4 * self.n * es, dtype=t.uint8, device=self.device)
+            self._ck(self.lib.rflbm_run_host(self.h, _ptr(rho_host), _ptr(u_host), int(nsteps), rho_out_host.data_ptr(),
+                                             u_out_host.data_ptr(), scratch.data_ptr(), scratch.numel()))
         return rho_out_host, u_out_host
+
+    # ---- slab faces (argument marshalling only; the CALLER moves the buffers between handles)
+    @property
+    def halo_bytes(self):
+        return int(self.lib.rflbm_halo_bytes(self.h))
+
+    @property
+    def halo_pending(self):
+        return bool(self.lib.rflbm_halo_pending(self.h))
+
+    def halo_pack(self, side, face=None):
+        with self._ctx():
+            if face is None:
+                face = self.torch.empty((9, self.ny, self.nx), dtype=self.dtype, device=self.device)
+            self._ck(self.lib.rflbm_halo_pack(self.h, int(side), face.data_ptr()))
+        return face
+
+    def halo_unpack(self, side, face):
+        with self._ctx():
+            assert face.dtype == self.dtype and face.numel() == 9 * self.nx * self.ny and face.is_contiguous()
+            self._ck(self.lib.rflbm_halo_unpack(self.h, int(side), face.data_ptr()))
+            self._keep_face = getattr(self, "_keep_face", {})
+            self._keep_face[side] = face
+
+    @property
+    def last_kernel(self):
+        return self.lib.rflbm_last_kernel(self.h).decode()
 
     @property
     def step_count(self):

@@ -1,7 +1,8 @@
 """Build the CUDA C-ABI library in-tree: paper_2507_08820_b200/csrc/librflbm.so (sm_100a only).
 
 nvcc cross-compiles without a GPU.  `python -m paper_2507_08820_b200.build` or build() from Python.
-The step kernels (~190 template instantiations) are compiled as six translation units, one per (precision, phase),
+The step kernels (~380 template instantiations) are compiled as 24 translation units, one per (precision, phase,
+tile width),
 in parallel with the C-ABI translation unit, then linked into one shared library.
 """
 from __future__ import annotations
@@ -20,8 +21,8 @@ HEADERS = ["rflbm_lattice.cuh", "rflbm_fastmath.cuh", "rflbm_rng.cuh", "rflbm_co
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC"]
 # (object name, source, extra defines)
 UNITS = [("rflbm.o", "rflbm.cu", [])] + [
-    (f"step_{r}_{p}.o", "rflbm_step_inst.cu", [f"-DRFLBM_INST_REAL={r}", f"-DRFLBM_INST_PHASE={p}"])
-    for r in ("double", "float") for p in (0, 1, 2)]
+    (f"step_{r}_{p}_{tx}.o", "rflbm_step_inst.cu", [f"-DRFLBM_INST_REAL={r}", f"-DRFLBM_INST_PHASE={p}", f"-DRFLBM_INST_TX={tx}"])
+    for tx in (128, 0, 64, 32) for r in ("double", "float") for p in (0, 1, 2)]
 
 
 def _stale() -> bool:

@@ -17,6 +17,17 @@ static size_t real_size(const rflbm* h) { return h->precision == RFLBM_F64 ? siz
 static size_t pop_bytes(const rflbm* h) { return (size_t)Q * (size_t)h->QS * real_size(h); }
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 static constexpr size_t TABLE_BYTES = (LOG_TABLE_N + SC_TABLE_N) * sizeof(f64x2);
+enum { HALO_NONE = 0, HALO_FILL = 1, HALO_HOME = 2 };
+
+// Storage layout.  Population arrays are NOT packed back to back: for power-of-two lattices
+// N*sizeof(real) is a power of two and the 27 read streams + 27 write streams of a step would all hit the same DRAM
+// channel/bank residues.  A pad of 37 x 256 B skews successive arrays; small lattices only round up to 32.
+static void set_layout(rflbm* h)
+{
+    const long long ns = (long long)h->px * h->ny * (h->nz + (h->slab ? 2 : 0));
+    const long long pad = (ns >= (1 << 16)) ? 37 * 32 : 0;
+    h->QS = (ns + 31) / 32 * 32 + pad;
+}
 
 static int fail(rflbm* h, int code, const char* fmt, ...)
 {
@@ -47,7 +58,7 @@ typedef CUresult (*encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_
                                     const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                     CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-// 4-D view [27][nz][ny][nx] of one population buffer, box = BOX_X consecutive x of one row of BOX_Q arrays
+// 4-D view [27][nzs][ny][nx] (row pitch px) of one population buffer, box = BOX_X consecutive x of one row of BOX_Q arrays
 static bool make_tensor_map(rflbm* h, void* base, CUtensorMap* out)
 {
     void* fn = nullptr;
@@ -57,11 +68,11 @@ static bool make_tensor_map(rflbm* h, void* base, CUtensorMap* out)
         cudaGetLastError();
         return false;
     }
-    const cuuint64_t dims[4] = {(cuuint64_t)h->nx, (cuuint64_t)h->ny, (cuuint64_t)h->nz, (cuuint64_t)Q};
     const bool f64 = h->precision == RFLBM_F64;
     const cuuint64_t es = f64 ? 8 : 4;
-    const cuuint64_t strides[3] = {(cuuint64_t)h->nx * es, (cuuint64_t)h->nx * h->ny * es, (cuuint64_t)h->QS * es};
-    const cuuint32_t box[4] = {(cuuint32_t)(f64 ? TmaGeom<double>::BOX_X : TmaGeom<float>::BOX_X), 1, 1, BOX_Q};   // 16-byte aligned starts
+    const cuuint64_t dims[4] = {(cuuint64_t)h->nx, (cuuint64_t)h->ny, (cuuint64_t)(h->nz + (h->slab ? 2 : 0)), (cuuint64_t)Q};
+    const cuuint64_t strides[3] = {(cuuint64_t)h->px * es, (cuuint64_t)h->px * h->ny * es, (cuuint64_t)h->QS * es};
+    const cuuint32_t box[4] = {(cuuint32_t)(h->tma_tx + 2 * (16 / (int)es)), 1, 1, BOX_Q};     // 16-byte aligned starts
     const cuuint32_t estr[4] = {1, 1, 1, 1};
     const CUresult r = ((encode_tiled_fn)fn)(out, f64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, base, dims, strides, box, estr,
                                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
@@ -76,36 +87,35 @@ extern "C" int rflbm_create(int nx, int ny, int nz, double tau, double kT, doubl
     *out = nullptr;
     if (nx < 1 || ny < 1 || nz < 1) return RFLBM_EINVAL;
     if ((double)nx * (double)ny * (double)nz >= 4294967296.0) return RFLBM_EINVAL;
-    if (ny > 65535 * 16 || nz > 65535) return RFLBM_EINVAL;
     if (!std::isfinite(tau) || !(tau > 0.5)) return RFLBM_EINVAL;
     if (!std::isfinite(kT) || kT < 0.0) return RFLBM_EINVAL;
     if (!std::isfinite(rho0) || !(rho0 > 0.0)) return RFLBM_EINVAL;
     if (precision != RFLBM_F64 && precision != RFLBM_F32) return RFLBM_EINVAL;
+    // one thread per site; a warp covers 32 consecutive x whenever nx >= 32
+    int bx = 8;
+    while (bx < nx && bx < 128) bx *= 2;
+    const int by = 128 / bx;
+    // gridDim.y / gridDim.z limits of the one-thread-per-site kernels (the TMA grid has fewer blocks in y)
+    if ((ny + by - 1) / by > 65535 || nz > 65535) return RFLBM_EINVAL;
     rflbm* h = new (std::nothrow) rflbm;
     if (!h) return RFLBM_ENOMEM;
     memset(h, 0, sizeof(*h));
     h->nx = nx; h->ny = ny; h->nz = nz;
     h->N = (long long)nx * ny * nz;
-    // Population arrays are NOT packed back to back: for power-of-two lattices N*sizeof(real) is a power of two
-    // and the 27 read streams + 27 write streams of a step would all hit the same DRAM channel/bank residues.
-    // A pad of 37 x 256 B skews successive arrays; small lattices only round up to 32.
-    long long pad = (h->N >= (1 << 16)) ? 37 * 32 : 0;
-    if (const char* e = getenv("RFLBM_QPAD")) pad = atoll(e) / 32 * 32;          // development knob (bench sweeps)
-    h->QS = (h->N + 31) / 32 * 32 + pad;
-    if ((double)h->QS >= 4294967296.0) { delete h; return RFLBM_EINVAL; }
     h->tau_g = 1.0;
     h->tau = tau; h->kT = kT; h->rho0 = rho0; h->seed = seed; h->precision = precision;
-    // one thread per site; a warp covers 32 consecutive x whenever nx >= 32
-    int bx = 8;
-    while (bx < nx && bx < 128) bx *= 2;
-    const int by = 128 / bx;
+    // internal row pitch: whole 128-byte lines per row, so that every lattice with nx >= 32 can take the TMA kernel
+    // (16-byte aligned box starts) and every warp's stores are line aligned; tiny lattices stay packed
+    const int line = 128 / (int)real_size(h);
+    h->px = (nx >= TMA_MIN_NX) ? (nx + line - 1) / line * line : nx;
+    h->tma_tx = nx >= 128 ? 128 : nx >= 64 ? 64 : nx >= TMA_MIN_NX ? 32 : 0;
+    set_layout(h);
+    if ((double)h->QS >= 4294967296.0) { delete h; return RFLBM_EINVAL; }
+    h->nzg = nz;
     h->block = dim3(bx, by, 1);
     h->grid = dim3((nx + bx - 1) / bx, (ny + by - 1) / by, nz);
     h->tma_rows = 16;
-    if (const char* e = getenv("RFLBM_TMA_ROWS")) {           // development knob (bench sweeps)
-        const int r = atoi(e);
-        if (r >= 1 && r <= 65536) h->tma_rows = r;
-    }
+    h->last_kernel = "";
     *out = h;
     return RFLBM_OK;
 }
@@ -134,16 +144,22 @@ extern "C" int rflbm_set_workspace(rflbm_t* h, void* dev_ptr, size_t bytes)
     h->aa_phase = 0;
     h->cur = 0;
     h->inited = false;
+    h->halo_mode = HALO_NONE;
+    h->halo_done = 0;
+    // The only device writes outside the handle's stream (include/rflbm.h says so): the scratch clear and the
+    // Box-Muller tables (host-generated, long double libm), both on the legacy stream, followed by a host-side wait
+    // for that stream: a pageable H2D copy may return before the DMA has landed and cudaMemset is asynchronous, and
+    // the kernels that read them run on h->stream, which need not be ordered against the legacy stream.
     if (int rc0 = check_cuda(h, cudaMemset(h->acc, 0, 4096), "scratch clear")) return rc0;
-    // the only device writes outside the stream: the scratch clear above and the Box-Muller tables
-    // (host-generated, long double libm)
     f64x2 host_tab[LOG_TABLE_N + SC_TABLE_N];                  // 12 KB on the stack: no shared state between handles
     fill_normal_tables(host_tab, host_tab + LOG_TABLE_N);
-    const int rc = check_cuda(h, cudaMemcpy(h->tables, host_tab, TABLE_BYTES, cudaMemcpyHostToDevice), "table upload");
+    int rc = check_cuda(h, cudaMemcpy(h->tables, host_tab, TABLE_BYTES, cudaMemcpyHostToDevice), "table upload");
     if (rc != RFLBM_OK) return rc;
-    // TMA path: rows of at least one 128-site tile, row pitch a multiple of 16 bytes (nx even for fp64, nx % 4 == 0 for fp32)
+    rc = check_cuda(h, cudaStreamSynchronize(0), "table upload (sync)");
+    if (rc != RFLBM_OK) return rc;
+    // TMA path: every lattice with nx >= 32 (rows of the internal buffers are 16-byte aligned by construction)
     h->tma_ok = false;
-    if (h->nx >= TMA_MIN_NX && h->nx % (16 / (int)real_size(h)) == 0)
+    if (h->tma_tx != 0)
         h->tma_ok = make_tensor_map(h, h->buf[0], &h->tmap[0]) && (nbuf == 1 || make_tensor_map(h, h->buf[1], &h->tmap[1]));
     return RFLBM_OK;
 }
@@ -158,7 +174,7 @@ extern "C" int rflbm_set_stream(rflbm_t* h, void* cuda_stream)
 extern "C" int rflbm_set_walls_z(rflbm_t* h, int on)
 {
     if (!h) return RFLBM_EINVAL;
-    if (on && h->nz < 3) return fail(h, RFLBM_EINVAL, "walls need nz >= 3");
+    if (on && (h->slab ? h->nzg : h->nz) < 3) return fail(h, RFLBM_EINVAL, "walls need nz >= 3");
     if (h->inited) return fail(h, RFLBM_ESTATE, "set_walls_z must precede init/set_populations");
     h->walls = on ? 1 : 0;
     return RFLBM_OK;
@@ -179,10 +195,10 @@ template <typename real>
 static FieldParams<real> field_params(const rflbm* h)
 {
     FieldParams<real> P;
-    P.nx = h->nx; P.ny = h->ny; P.nz = h->nz; P.N = h->N; P.QS = h->QS;
+    P.G = make_geom(h);
     P.hgx = (real)(0.5 * h->g[0]); P.hgy = (real)(0.5 * h->g[1]); P.hgz = (real)(0.5 * h->g[2]);
-    P.walls = h->walls;
     P.aa = (h->scheme == RFLBM_SCHEME_AA) ? 1 : 0;
+    P.ghost_in = h->slab ? 1 : 0;
     return P;
 }
 
@@ -191,7 +207,7 @@ static StepParams<real> step_params(const rflbm* h, uint64_t t)
 {
     StepParams<real> P;
     const double omega = 1.0 / h->tau;
-    P.nx = h->nx; P.ny = h->ny; P.nz = h->nz; P.N = h->N; P.QS = h->QS;
+    P.G = make_geom(h);
     P.half_omc = (real)(0.5 * (1.0 - omega));
     const double omega_g = 1.0 / h->tau_g;
     P.omc_g = (real)(1.0 - omega_g);
@@ -234,6 +250,21 @@ static int gather_mode(const rflbm* h)
         }                                                                                                         \
     } while (0)
 
+// slab mode: what the next halo exchange has to carry
+//   A-B, and AA after an even step: the ghost layers must receive the neighbours' face populations before the next
+//   pull (HALO_FILL); AA after an odd step: the ghost layers hold what this slab pushed across its faces and the
+//   neighbours have to take it home (HALO_HOME); AA in the natural layout with nothing pushed yet: nothing.
+static void after_state_change(rflbm* h)
+{
+    h->halo_done = 0;
+    if (!h->slab) h->halo_mode = HALO_NONE;
+    else if (h->scheme == RFLBM_SCHEME_AB) h->halo_mode = HALO_FILL;
+    else h->halo_mode = HALO_NONE;                 // AA after init / set_populations; rflbm_step sets it afterwards
+}
+static bool halo_pending(const rflbm* h) { return h->slab && h->halo_mode != HALO_NONE && h->halo_done != 3; }
+#define RFLBM_REQUIRE_HALO(h)                                                                                    \
+    if (halo_pending(h)) return fail(h, RFLBM_ESTATE, "slab: halo exchange pending (rflbm_halo_pack / rflbm_halo_unpack on both sides)")
+
 // ---------------------------------------------------------------- init / import / export
 template <typename real>
 static int do_init(rflbm* h, const void* rho, const void* u)
@@ -259,6 +290,7 @@ extern "C" int rflbm_init(rflbm_t* h, const void* rho_dev, const void* u_dev)
     h->aa_phase = 0;
     h->t = 0;
     h->inited = true;
+    after_state_change(h);
     return RFLBM_OK;
 }
 
@@ -284,6 +316,7 @@ extern "C" int rflbm_set_populations(rflbm_t* h, const void* f_dev, uint64_t ste
     h->aa_phase = 0;
     h->t = step;
     h->inited = true;
+    after_state_change(h);
     return RFLBM_OK;
 }
 
@@ -300,6 +333,7 @@ extern "C" int rflbm_get_populations(rflbm_t* h, void* f_dev)
     if (!h) return RFLBM_EINVAL;
     if (!f_dev) return fail(h, RFLBM_EINVAL, "f_dev is NULL");
     if (!h->inited) return fail(h, RFLBM_ESTATE, "rflbm_get_populations before init");
+    RFLBM_REQUIRE_HALO(h);
     return (h->precision == RFLBM_F64) ? do_export<double>(h, f_dev) : do_export<float>(h, f_dev);
 }
 
@@ -312,20 +346,34 @@ static bool use_tma(const rflbm* h)
     return h->variant == RFLBM_KERNEL_TMA || h->kT > 0.0;
 }
 
-// the step kernels are instantiated in rflbm_step_inst.cu, one translation unit per (precision, phase)
-extern template void dispatch_variant<double, STEP_AB>(rflbm*, const StepParams<double>&, int, bool);
-extern template void dispatch_variant<double, STEP_AA_EVEN>(rflbm*, const StepParams<double>&, int, bool);
-extern template void dispatch_variant<double, STEP_AA_ODD>(rflbm*, const StepParams<double>&, int, bool);
-extern template void dispatch_variant<float, STEP_AB>(rflbm*, const StepParams<float>&, int, bool);
-extern template void dispatch_variant<float, STEP_AA_EVEN>(rflbm*, const StepParams<float>&, int, bool);
-extern template void dispatch_variant<float, STEP_AA_ODD>(rflbm*, const StepParams<float>&, int, bool);
+// the step kernels are instantiated in rflbm_step_inst.cu, one translation unit per (precision, phase, tile width)
+#define RFLBM_EXTERN_INST(R, PH)                                                                     \
+    extern template void dispatch_variant<R, PH, 0>(rflbm*, const StepParams<R>&, int);              \
+    extern template void dispatch_variant<R, PH, 32>(rflbm*, const StepParams<R>&, int);             \
+    extern template void dispatch_variant<R, PH, 64>(rflbm*, const StepParams<R>&, int);             \
+    extern template void dispatch_variant<R, PH, 128>(rflbm*, const StepParams<R>&, int);
+RFLBM_EXTERN_INST(double, STEP_AB)
+RFLBM_EXTERN_INST(double, STEP_AA_EVEN)
+RFLBM_EXTERN_INST(double, STEP_AA_ODD)
+RFLBM_EXTERN_INST(float, STEP_AB)
+RFLBM_EXTERN_INST(float, STEP_AA_EVEN)
+RFLBM_EXTERN_INST(float, STEP_AA_ODD)
+
+template <typename real, int PHASE>
+static void dispatch_tile(rflbm* h, const StepParams<real>& P, int variant, int tx)
+{
+    if (tx == 128) dispatch_variant<real, PHASE, 128>(h, P, variant);
+    else if (tx == 64) dispatch_variant<real, PHASE, 64>(h, P, variant);
+    else if (tx == 32) dispatch_variant<real, PHASE, 32>(h, P, variant);
+    else dispatch_variant<real, PHASE, 0>(h, P, variant);
+}
 
 template <typename real>
-static void dispatch_step(rflbm* h, const StepParams<real>& P, int variant, bool tma)
+static void dispatch_step(rflbm* h, const StepParams<real>& P, int variant, int tx)
 {
-    if (h->scheme == RFLBM_SCHEME_AB) dispatch_variant<real, STEP_AB>(h, P, variant, tma);
-    else if (h->aa_phase == 0) dispatch_variant<real, STEP_AA_EVEN>(h, P, variant, tma);
-    else dispatch_variant<real, STEP_AA_ODD>(h, P, variant, tma);
+    if (h->scheme == RFLBM_SCHEME_AB) dispatch_tile<real, STEP_AB>(h, P, variant, tx);
+    else if (h->aa_phase == 0) dispatch_tile<real, STEP_AA_EVEN>(h, P, variant, tx);
+    else dispatch_tile<real, STEP_AA_ODD>(h, P, variant, tx);
 }
 
 template <typename real>
@@ -333,18 +381,24 @@ static int do_step(rflbm* h, int nsteps)
 {
     const bool noise = h->kT > 0.0;       // kT = 0: deterministic (Reg-)LBM, RNG skipped entirely (R17)
     if (h->variant == RFLBM_KERNEL_TMA && !h->tma_ok)
-        return fail(h, RFLBM_EINVAL, "TMA kernel needs nx >= 128 and a row pitch that is a multiple of 16 bytes");
+        return fail(h, RFLBM_EINVAL, "the TMA kernel needs nx >= 32 (and a driver that exports cuTensorMapEncodeTiled)");
     const bool tma = use_tma(h);
     const bool ghost = h->model == RFLBM_MODEL_REG && h->tau_g != 1.0;
     const int variant = (ghost ? 16 : 0) | (h->model == RFLBM_MODEL_BGK ? 8 : 0) | (h->walls ? 4 : 0) | (h->force ? 2 : 0) | (noise ? 1 : 0);
+    static const char* const names[4] = {"step_kernel", "step_kernel_tma<TX=32>", "step_kernel_tma<TX=64>", "step_kernel_tma<TX=128>"};
     for (int s = 0; s < nsteps; ++s) {
         const StepParams<real> P = step_params<real>(h, h->t);
-        dispatch_step<real>(h, P, variant, tma);
-        const int rc = after_launch(h, tma ? "step_kernel_tma" : "step_kernel");
+        dispatch_step<real>(h, P, variant, tma ? h->tma_tx : 0);
+        h->last_kernel = !tma ? names[0] : h->tma_tx == 32 ? names[1] : h->tma_tx == 64 ? names[2] : names[3];
+        const int rc = after_launch(h, h->last_kernel);
         if (rc != RFLBM_OK) return rc;
         if (h->scheme == RFLBM_SCHEME_AB) h->cur ^= 1;
         else h->aa_phase ^= 1;
         h->t += 1;
+        if (h->slab) {
+            h->halo_done = 0;
+            h->halo_mode = (h->scheme == RFLBM_SCHEME_AB || h->aa_phase == 1) ? HALO_FILL : HALO_HOME;
+        }
     }
     return RFLBM_OK;
 }
@@ -354,6 +408,8 @@ extern "C" int rflbm_step(rflbm_t* h, int nsteps)
     if (!h) return RFLBM_EINVAL;
     if (nsteps < 0) return fail(h, RFLBM_EINVAL, "nsteps < 0");
     if (!h->inited) return fail(h, RFLBM_ESTATE, "rflbm_step before init");
+    if (h->slab && nsteps > 1) return fail(h, RFLBM_EINVAL, "slab: one step at a time (the halos are exchanged between steps)");
+    if (nsteps > 0) RFLBM_REQUIRE_HALO(h);
     return (h->precision == RFLBM_F64) ? do_step<double>(h, nsteps) : do_step<float>(h, nsteps);
 }
 
@@ -371,6 +427,7 @@ extern "C" int rflbm_moments(rflbm_t* h, void* rho_dev, void* u_dev)
     if (!h) return RFLBM_EINVAL;
     if (!rho_dev || !u_dev) return fail(h, RFLBM_EINVAL, "rho_dev / u_dev is NULL");
     if (!h->inited) return fail(h, RFLBM_ESTATE, "rflbm_moments before init");
+    RFLBM_REQUIRE_HALO(h);
     return (h->precision == RFLBM_F64) ? do_moments<double>(h, rho_dev, u_dev) : do_moments<float>(h, rho_dev, u_dev);
 }
 
@@ -387,6 +444,7 @@ extern "C" int rflbm_stress(rflbm_t* h, void* pi_dev)
     if (!h) return RFLBM_EINVAL;
     if (!pi_dev) return fail(h, RFLBM_EINVAL, "pi_dev is NULL");
     if (!h->inited) return fail(h, RFLBM_ESTATE, "rflbm_stress before init");
+    RFLBM_REQUIRE_HALO(h);
     return (h->precision == RFLBM_F64) ? do_stress<double>(h, pi_dev) : do_stress<float>(h, pi_dev);
 }
 
@@ -403,6 +461,7 @@ extern "C" int rflbm_diagnostics(rflbm_t* h, double out_host[10])
     if (!h) return RFLBM_EINVAL;
     if (!out_host) return fail(h, RFLBM_EINVAL, "out_host is NULL");
     if (!h->inited) return fail(h, RFLBM_ESTATE, "rflbm_diagnostics before init");
+    RFLBM_REQUIRE_HALO(h);
     int rc = check_cuda(h, cudaMemsetAsync(h->acc, 0, 10 * sizeof(double), h->stream), "cudaMemsetAsync");
     if (rc != RFLBM_OK) return rc;
     rc = (h->precision == RFLBM_F64) ? do_diagnostics<double>(h) : do_diagnostics<float>(h);
@@ -412,7 +471,10 @@ extern "C" int rflbm_diagnostics(rflbm_t* h, double out_host[10])
     if (rc != RFLBM_OK) return rc;
     rc = check_cuda(h, cudaStreamSynchronize(h->stream), "cudaStreamSynchronize");
     if (rc != RFLBM_OK) return rc;
-    const double nf = (double)h->nx * h->ny * (h->walls ? h->nz - 2 : h->nz);
+    // fluid layers owned by this handle (solid layers are global z = 0 and nz_global - 1)
+    const int z0 = h->slab ? h->z0 : 0, nzg = h->slab ? h->nzg : h->nz;
+    const int nfl = h->nz - (h->walls ? (z0 == 0) + (z0 + h->nz == nzg) : 0);
+    const double nf = (double)h->nx * h->ny * nfl;
     out_host[0] = s[0];
     for (int a = 0; a < 3; ++a) {
         out_host[1 + a] = s[1 + a];
@@ -459,6 +521,7 @@ extern "C" int rflbm_run_host(rflbm_t* h, const void* rho_host, const void* u_ho
     if (!rho_out_host || !u_out_host || !scratch_dev) return fail(h, RFLBM_EINVAL, "NULL output or scratch pointer");
     if ((rho_host == nullptr) != (u_host == nullptr))
         return fail(h, RFLBM_EINVAL, "rho_host and u_host must both be given or both NULL");
+    if (h->slab) return fail(h, RFLBM_ESTATE, "rflbm_run_host is a whole-lattice job: not available in slab mode");
     const size_t fb = (size_t)h->N * real_size(h);
     if (scratch_bytes < 4 * fb) return fail(h, RFLBM_ENOMEM, "scratch too small: %zu < %zu bytes", scratch_bytes, 4 * fb);
     char* d_rho = (char*)scratch_dev;
@@ -494,6 +557,91 @@ extern "C" int rflbm_set_scheme(rflbm_t* h, int scheme)
     return RFLBM_OK;
 }
 
+// ---------------------------------------------------------------- z-slab decomposition
+extern "C" int rflbm_set_slab(rflbm_t* h, int z0, int nz_global)
+{
+    if (!h) return RFLBM_EINVAL;
+    if (h->ws) return fail(h, RFLBM_ESTATE, "rflbm_set_slab must precede rflbm_set_workspace (the workspace size depends on it)");
+    if (z0 < 0 || nz_global < 1 || (long long)z0 + h->nz > nz_global)
+        return fail(h, RFLBM_EINVAL, "slab [%d, %d) does not fit in %d global layers", z0, z0 + h->nz, nz_global);
+    if ((double)h->nx * (double)h->ny * (double)nz_global >= 4294967296.0)
+        return fail(h, RFLBM_EINVAL, "global lattice has 2^32 sites or more (the Philox site key is 32 bits, R8)");
+    if (h->walls && nz_global < 3) return fail(h, RFLBM_EINVAL, "walls need nz_global >= 3");
+    const int was = h->slab, was_z0 = h->z0, was_nzg = h->nzg;
+    h->slab = 1; h->z0 = z0; h->nzg = nz_global;
+    set_layout(h);
+    if ((double)h->QS >= 4294967296.0) {
+        h->slab = was; h->z0 = was_z0; h->nzg = was_nzg;
+        set_layout(h);
+        return fail(h, RFLBM_EINVAL, "slab too large");
+    }
+    return RFLBM_OK;
+}
+
+extern "C" size_t rflbm_halo_bytes(const rflbm_t* h)
+{
+    return h ? (size_t)9 * (size_t)h->nx * (size_t)h->ny * real_size(h) : 0;
+}
+
+extern "C" int rflbm_halo_pending(const rflbm_t* h) { return (h && halo_pending(h)) ? 1 : 0; }
+
+// which storage layer and which 9 consecutive slots a face call touches (rflbm_kernels.cuh::halo_kernel).
+// Storage layers: 0 = ghost below, 1..nz = owned, nz+1 = ghost above.  Slots 0..8 have c_z = -1, 18..26 c_z = +1.
+//   HALO_FILL, A-B : the neighbour below pulls slot q (c_z = -1) of my bottom layer through its upper ghost
+//   HALO_FILL, AA  : ... slot 26-q instead, i.e. the other nine
+//   HALO_HOME (AA after an odd step): my lower ghost holds the c_z = -1 populations my bottom layer pushed down; they
+//                    belong in slot q of the top layer of the neighbour below (and mirrored for the upper face)
+// A buffer packed on one side is unpacked on the OTHER side of the neighbour with the same slots.
+struct HaloPlan { int z, slot0; bool skip; };
+static HaloPlan halo_plan(const rflbm* h, int side, bool pack)
+{
+    const bool ab = h->scheme == RFLBM_SCHEME_AB, low = side == RFLBM_SIDE_LOW;
+    HaloPlan p;
+    p.skip = false;
+    if (h->halo_mode == HALO_FILL) {
+        if (pack) { p.z = low ? 1 : h->nz; p.slot0 = (low == ab) ? 0 : 18; }
+        else { p.z = low ? 0 : h->nz + 1; p.slot0 = (low == ab) ? 18 : 0; }
+    } else {
+        if (pack) { p.z = low ? 0 : h->nz + 1; p.slot0 = low ? 0 : 18; }
+        else {
+            p.z = low ? 1 : h->nz; p.slot0 = low ? 18 : 0;
+            // nothing crosses a face next to a solid layer: a solid layer is never updated (it pushed nothing, and
+            // keeps its values), and the fluid layer beside it bounced its populations back instead of pushing them
+            const int zt = h->z0 + (low ? 0 : h->nz - 1);                                  // receiving layer
+            const int zf = (zt + (low ? -1 : 1) + h->nzg) % h->nzg;                        // layer the data would come from
+            p.skip = h->walls && (zt == 0 || zt == h->nzg - 1 || zf == 0 || zf == h->nzg - 1);
+        }
+    }
+    return p;
+}
+
+template <bool PACK>
+static int do_halo(rflbm* h, int side, void* face_dev)
+{
+    if (!h) return RFLBM_EINVAL;
+    if (side != RFLBM_SIDE_LOW && side != RFLBM_SIDE_HIGH) return fail(h, RFLBM_EINVAL, "unknown side %d", side);
+    if (!face_dev) return fail(h, RFLBM_EINVAL, "face_dev is NULL");
+    if (!h->slab) return fail(h, RFLBM_ESTATE, "not in slab mode (rflbm_set_slab)");
+    if (!h->inited) return fail(h, RFLBM_ESTATE, "halo call before init");
+    if (h->halo_mode == HALO_NONE || (PACK && h->halo_done == 3)) return RFLBM_OK;    // nothing to exchange in this state
+    const HaloPlan p = halo_plan(h, side, PACK);
+    if (!p.skip) {
+        const Geom G = make_geom(h);
+        const dim3 grid(h->grid.x, h->grid.y, 1);
+        if (h->precision == RFLBM_F64)
+            halo_kernel<double, PACK><<<grid, h->block, 0, h->stream>>>((double*)h->buf[h->cur], (double*)face_dev, G, p.z, p.slot0);
+        else
+            halo_kernel<float, PACK><<<grid, h->block, 0, h->stream>>>((float*)h->buf[h->cur], (float*)face_dev, G, p.z, p.slot0);
+        const int rc = after_launch(h, PACK ? "halo_kernel<pack>" : "halo_kernel<unpack>");
+        if (rc != RFLBM_OK) return rc;
+    }
+    if (!PACK) h->halo_done |= (side == RFLBM_SIDE_LOW) ? 1 : 2;
+    return RFLBM_OK;
+}
+
+extern "C" int rflbm_halo_pack(rflbm_t* h, int side, void* face_dev) { return do_halo<true>(h, side, face_dev); }
+extern "C" int rflbm_halo_unpack(rflbm_t* h, int side, const void* face_dev) { return do_halo<false>(h, side, const_cast<void*>(face_dev)); }
+
 extern "C" int rflbm_set_ghost_tau(rflbm_t* h, double tau_g)
 {
     if (!h) return RFLBM_EINVAL;
@@ -523,6 +671,7 @@ extern "C" int rflbm_set_kernel_variant(rflbm_t* h, int variant)
 
 // ---------------------------------------------------------------- misc
 extern "C" uint64_t rflbm_launch_count(const rflbm_t* h) { return h ? h->launches : 0; }
+extern "C" const char* rflbm_last_kernel(const rflbm_t* h) { return h ? h->last_kernel : ""; }
 extern "C" uint64_t rflbm_step_count(const rflbm_t* h) { return h ? h->t : 0; }
 extern "C" const char* rflbm_last_error(const rflbm_t* h) { return h ? h->err : "NULL handle"; }
 

@@ -35,11 +35,25 @@ __host__ __device__ constexpr int amp_class(int p, int q, int r)
          : (n2 == 2 && n1 == 1) ? AMP_221 : AMP_222;
 }
 
+// Geometry of one handle.  Logical lattice nx x ny x nz ("owned" layers); the internal buffers
+// have a row pitch px >= nx (rows 16-byte aligned so that every lattice can take the TMA kernel) and, in slab mode
+// (rflbm_set_slab), one ghost layer below and above the owned layers.  Walls and the Philox site key use GLOBAL z.
+struct Geom {
+    int nx, ny;             // logical extent in x, y (periodic)
+    int nz;                 // owned layers
+    int nzs;                // layers in storage: nz, or nz + 2 in slab mode
+    int z_lo;               // storage index of the first owned layer: 0, or 1 in slab mode
+    int zg0;                // global z of storage layer 0: 0, or z0 - 1 in slab mode
+    int nzg;                // global number of layers (= nz without a slab)
+    int px;                 // row pitch of the internal buffers, in elements
+    long long pxy;          // px * ny
+    long long QS;           // elements between consecutive population arrays inside a buffer
+    long long N;            // nx * ny * nz: length of the canonical (boundary) arrays
+};
+
 template <typename real>
 struct StepParams {
-    int nx, ny, nz;
-    long long N;
-    long long QS;           // elements between consecutive population arrays (N + padding, see rflbm.cu)
+    Geom G;
     real half_omc;          // (1 - omega_h)/2
     real omc_g;             // 1 - omega_g (0 in the paper's final scheme, :215)
     real amp[AMP_N];        // noise amplitude per class (times sqrt(rho) at the site), Eq.9

@@ -1,35 +1,46 @@
 // rflbm_kernels.cuh — CUDA kernels of the Reg-FLBM path (sm_100a).
 //
-// Storage: SoA buffers P[q][z][y][x] of `real` in the lex order of rflbm_lattice.cuh, the 27
-// arrays QS elements apart.
+// Storage: SoA buffers P[q][z][y][x] of `real` in the lex order of rflbm_lattice.cuh, rows
+// px >= nx elements apart (16-byte aligned rows whatever nx is), the 27 arrays QS elements apart.
 //   A-B scheme: two buffers holding POST-collision, UN-streamed populations (R10).  A step PULLS
 //     S_t[q](x) = P_{t-1}[q](x - c_q)  (Eq.7 :87; bounce-back: P_{t-1}[26-q](x) when x - c_q is solid, R12),
 //     collides in registers and stores P_t[q](x): 27 neighbour reads (coalesced, at most one element off alignment)
 //     and 27 aligned coalesced writes per site, nothing else.
 //   AA scheme: one buffer updated in place, alternating an all-local step and a pull/push step (STEP_AA_EVEN/ODD).
 // The observables gather the pre-collision state S_t according to scheme and phase (GATHER_*).
+// Slab mode (rflbm_set_slab; "linear decomposition" along z): the buffers carry one ghost layer
+// below and above the owned layers, filled by the halo calls; nothing wraps in z, and the solid-layer test and the
+// Philox site key use the GLOBAL z, so a slab computes exactly what the undivided lattice computes there.
 #pragma once
 #include "rflbm_collide.cuh"
 
 namespace rflbm_dev {
 
 struct SiteIndex {
-    int x, y, z;
+    int x, y, z;        // z: storage layer
+    int zg;             // global layer (walls, RNG key)
     bool valid;
-    long long s;        // x + nx (y + ny z)
+    long long s;        // storage index  x + px (y + ny z)
+    long long sl;       // canonical index x + nx (y + ny (z - z_lo)) of the boundary arrays
+    uint32_t site;      // Philox key     x + nx (y + ny zg)  (R8; < 2^32 by rflbm_create / rflbm_set_slab)
 };
 
 // one thread per site: blockDim = (bx, by), grid = (ceil(nx/bx), ceil(ny/by), nz)
-__device__ __forceinline__ SiteIndex my_site(int nx, int ny)
+__device__ __forceinline__ SiteIndex my_site(const Geom& G)
 {
     SiteIndex i;
     i.x = blockIdx.x * blockDim.x + threadIdx.x;
     i.y = blockIdx.y * blockDim.y + threadIdx.y;
-    i.z = blockIdx.z;
-    i.valid = (i.x < nx) && (i.y < ny);
-    i.s = (long long)i.x + (long long)nx * ((long long)i.y + (long long)ny * (long long)i.z);
+    i.z = (int)blockIdx.z + G.z_lo;
+    i.zg = i.z + G.zg0;
+    i.valid = (i.x < G.nx) && (i.y < G.ny);
+    i.s = (long long)i.x + (long long)G.px * i.y + G.pxy * i.z;
+    i.sl = (long long)i.x + (long long)G.nx * ((long long)i.y + (long long)G.ny * (long long)blockIdx.z);
+    i.site = (uint32_t)((long long)i.x + (long long)G.nx * ((long long)i.y + (long long)G.ny * (long long)i.zg));
     return i;
 }
+
+__device__ __forceinline__ bool solid_layer(const Geom& G, int zg) { return zg == 0 || zg == G.nzg - 1; }
 
 // Where the pre-collision population S_t[q](x) of a site sits in the buffer:
 //   GATHER_AB   A-B scheme: slot q of the neighbour x - c_q   (bounce-back: slot 26-q of the site itself)
@@ -40,32 +51,32 @@ enum { GATHER_AB = 0, GATHER_AA1 = 1, GATHER_AA0 = 2 };
 
 // Gather of the 27 pre-collision populations of a site into g[cz+1][cy+1][cx+1].
 template <typename real, bool WALLS, int MODE = GATHER_AB>
-__device__ __forceinline__ void gather(const real* __restrict__ src, long long QS, int nx, int ny, int nz,
-                                       const SiteIndex& i, real (&g)[3][3][3])
+__device__ __forceinline__ void gather(const real* __restrict__ src, const Geom& G, const SiteIndex& i, real (&g)[3][3][3])
 {
     if (MODE == GATHER_AA0) {
 #pragma unroll
-        for (int q = 0; q < Q; ++q) g[q / 9][(q / 3) % 3][q % 3] = src[(long long)q * QS + i.s];   // in-place buffer: no LDG.NC
+        for (int q = 0; q < Q; ++q) g[q / 9][(q / 3) % 3][q % 3] = src[(long long)q * G.QS + i.s];   // in-place buffer: no LDG.NC
         return;
     }
-    // neighbour coordinates x - cx etc. with periodic wrap; index a = cx+1 reads from xs[a]
-    const int xs[3] = {(i.x + 1 == nx) ? 0 : i.x + 1, i.x, (i.x == 0) ? nx - 1 : i.x - 1};
-    const int ys[3] = {(i.y + 1 == ny) ? 0 : i.y + 1, i.y, (i.y == 0) ? ny - 1 : i.y - 1};
-    const int zs[3] = {(i.z + 1 == nz) ? 0 : i.z + 1, i.z, (i.z == 0) ? nz - 1 : i.z - 1};
+    // neighbour coordinates x - cx etc. with periodic wrap; index a = cx+1 reads from xs[a].  In slab mode the ghost
+    // layers make the z wrap unreachable (owned layers are 1..nzs-2).
+    const int xs[3] = {(i.x + 1 == G.nx) ? 0 : i.x + 1, i.x, (i.x == 0) ? G.nx - 1 : i.x - 1};
+    const int ys[3] = {(i.y + 1 == G.ny) ? 0 : i.y + 1, i.y, (i.y == 0) ? G.ny - 1 : i.y - 1};
+    const int zs[3] = {(i.z + 1 == G.nzs) ? 0 : i.z + 1, i.z, (i.z == 0) ? G.nzs - 1 : i.z - 1};
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        // with walls the fluid layers are z = 1..nz-2; x - c_q is solid iff (cz=+1 and z==1) or (cz=-1 and z==nz-2)
-        const bool bounce = WALLS && ((c == 2 && i.z == 1) || (c == 0 && i.z == nz - 2));
+        // with walls the fluid layers are zg = 1..nzg-2; x - c_q is solid iff (cz=+1 and zg==1) or (cz=-1 and zg==nzg-2)
+        const bool bounce = WALLS && ((c == 2 && i.zg == 1) || (c == 0 && i.zg == G.nzg - 2));
 #pragma unroll
         for (int b = 0; b < 3; ++b) {
-            const long long row = (long long)nx * ((long long)ys[b] + (long long)ny * (long long)zs[c]);
+            const long long row = (long long)G.px * ys[b] + G.pxy * zs[c];
 #pragma unroll
             for (int a = 0; a < 3; ++a) {
                 const int q = a + 3 * b + 9 * c;
                 const int slot_pull = (MODE == GATHER_AA1) ? 26 - q : q;
                 const int slot_back = (MODE == GATHER_AA1) ? q : 26 - q;
-                const long long pull = (long long)slot_pull * QS + row + xs[a];
-                const long long back = (long long)slot_back * QS + i.s;
+                const long long pull = (long long)slot_pull * G.QS + row + xs[a];
+                const long long back = (long long)slot_back * G.QS + i.s;
                 const long long at = (WALLS && bounce) ? back : pull;
                 g[c][b][a] = (MODE == GATHER_AB) ? __ldg(src + at) : src[at];     // AA: the buffer is written in place
             }
@@ -93,31 +104,31 @@ __device__ __forceinline__ void stage_tables(const f64x2* __restrict__ tab, f64x
 enum { STEP_AB = 0, STEP_AA_EVEN = 1, STEP_AA_ODD = 2 };
 
 template <typename real, bool WALLS, int PHASE>
-__device__ __forceinline__ void scatter(real* dst, long long QS, int nx, int ny, int nz, const SiteIndex& i,
-                                        const real (&g)[3][3][3])
+__device__ __forceinline__ void scatter(real* dst, const Geom& G, const SiteIndex& i, const real (&g)[3][3][3])
 {
     if (PHASE != STEP_AA_ODD) {
 #pragma unroll
         for (int q = 0; q < Q; ++q)
-            __stcs(dst + (long long)((PHASE == STEP_AA_EVEN) ? 26 - q : q) * QS + i.s, g[q / 9][(q / 3) % 3][q % 3]);
+            __stcs(dst + (long long)((PHASE == STEP_AA_EVEN) ? 26 - q : q) * G.QS + i.s, g[q / 9][(q / 3) % 3][q % 3]);
         return;
     }
-    // push: x + c_q with periodic wrap; index a = cx+1 writes to xd[a]
-    const int xd[3] = {(i.x == 0) ? nx - 1 : i.x - 1, i.x, (i.x + 1 == nx) ? 0 : i.x + 1};
-    const int yd[3] = {(i.y == 0) ? ny - 1 : i.y - 1, i.y, (i.y + 1 == ny) ? 0 : i.y + 1};
-    const int zd[3] = {(i.z == 0) ? nz - 1 : i.z - 1, i.z, (i.z + 1 == nz) ? 0 : i.z + 1};
+    // push: x + c_q with periodic wrap; index a = cx+1 writes to xd[a] (slab mode: the ghost layers take the z = -1
+    // and z = nz pushes, rflbm_halo_* carry them home)
+    const int xd[3] = {(i.x == 0) ? G.nx - 1 : i.x - 1, i.x, (i.x + 1 == G.nx) ? 0 : i.x + 1};
+    const int yd[3] = {(i.y == 0) ? G.ny - 1 : i.y - 1, i.y, (i.y + 1 == G.ny) ? 0 : i.y + 1};
+    const int zd[3] = {(i.z == 0) ? G.nzs - 1 : i.z - 1, i.z, (i.z + 1 == G.nzs) ? 0 : i.z + 1};
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        // x + c_q is solid iff (cz=-1 and z==1) or (cz=+1 and z==nz-2): the population returns to the site as 26-q
-        const bool bounce = WALLS && ((c == 0 && i.z == 1) || (c == 2 && i.z == nz - 2));
+        // x + c_q is solid iff (cz=-1 and zg==1) or (cz=+1 and zg==nzg-2): the population returns to the site as 26-q
+        const bool bounce = WALLS && ((c == 0 && i.zg == 1) || (c == 2 && i.zg == G.nzg - 2));
 #pragma unroll
         for (int b = 0; b < 3; ++b) {
-            const long long row = (long long)nx * ((long long)yd[b] + (long long)ny * (long long)zd[c]);
+            const long long row = (long long)G.px * yd[b] + G.pxy * zd[c];
 #pragma unroll
             for (int a = 0; a < 3; ++a) {
                 const int q = a + 3 * b + 9 * c;
-                const long long push = (long long)q * QS + row + xd[a];
-                const long long back = (long long)(26 - q) * QS + i.s;
+                const long long push = (long long)q * G.QS + row + xd[a];
+                const long long back = (long long)(26 - q) * G.QS + i.s;
                 __stcs(dst + ((WALLS && bounce) ? back : push), g[c][b][a]);
             }
         }
@@ -131,45 +142,43 @@ step_kernel(const real* src, real* dst, const __grid_constant__ StepParams<real>
     constexpr bool TABLES = NOISE && sizeof(real) == 8;
     __shared__ f64x2 s_tab[TABLES ? LOG_TABLE_N + SC_TABLE_N : 1];
     if (TABLES) stage_tables(P.tables, s_tab);
-    const SiteIndex i = my_site(P.nx, P.ny);
+    const SiteIndex i = my_site(P.G);
     if (!i.valid) return;
-    if (WALLS && (i.z == 0 || i.z == P.nz - 1)) return;    // solid layers are never updated
+    if (WALLS && solid_layer(P.G, i.zg)) return;           // solid layers are never updated
     real g[3][3][3];
-    gather<real, WALLS, PHASE == STEP_AB ? GATHER_AB : PHASE == STEP_AA_EVEN ? GATHER_AA0 : GATHER_AA1>(
-        src, P.QS, P.nx, P.ny, P.nz, i, g);
-    collide<real, FORCE, NOISE, BGK, GHOST>(g, P, (uint32_t)i.s, s_tab, s_tab + LOG_TABLE_N);
-    scatter<real, WALLS, PHASE>(dst, P.QS, P.nx, P.ny, P.nz, i, g);
+    gather<real, WALLS, PHASE == STEP_AB ? GATHER_AB : PHASE == STEP_AA_EVEN ? GATHER_AA0 : GATHER_AA1>(src, P.G, i, g);
+    collide<real, FORCE, NOISE, BGK, GHOST>(g, P, i.site, s_tab, s_tab + LOG_TABLE_N);
+    scatter<real, WALLS, PHASE>(dst, P.G, i, g);
 }
 
 // ---------------------------------------------------------------- observables
 template <typename real>
 struct FieldParams {
-    int nx, ny, nz;
-    long long N;
-    long long QS;         // elements between consecutive population arrays of the internal storage (>= N)
+    Geom G;
     real hgx, hgy, hgz;   // g/2: reported velocity u = j/rho + g/2 (R13)
-    int walls;
     int aa;               // AA scheme: one buffer in the natural layout P[q](s) = S[q](s) at even phase
+    int ghost_in;         // slab mode: the fields given to init / set_populations carry one extra layer below and above
 };
 
 template <typename real, bool WALLS, int MODE>
 __global__ void __launch_bounds__(128)
 moments_kernel(const real* __restrict__ src, real* __restrict__ rho, real* __restrict__ u, const FieldParams<real> P)
 {
-    const SiteIndex i = my_site(P.nx, P.ny);
+    const SiteIndex i = my_site(P.G);
     if (!i.valid) return;
-    if (WALLS && (i.z == 0 || i.z == P.nz - 1)) {
-        rho[i.s] = real(0); u[i.s] = real(0); u[P.N + i.s] = real(0); u[2 * P.N + i.s] = real(0);
+    const long long N = P.G.N;
+    if (WALLS && solid_layer(P.G, i.zg)) {
+        rho[i.sl] = real(0); u[i.sl] = real(0); u[N + i.sl] = real(0); u[2 * N + i.sl] = real(0);
         return;
     }
     real g[3][3][3];
-    gather<real, WALLS, MODE>(src, P.QS, P.nx, P.ny, P.nz, i, g);
+    gather<real, WALLS, MODE>(src, P.G, i, g);
     const Moments10<real> m = forward_moments(g);
     const real inv = real(1.0) / m.rho;
-    rho[i.s] = m.rho;
-    u[i.s] = fma(m.jx, inv, P.hgx);
-    u[P.N + i.s] = fma(m.jy, inv, P.hgy);
-    u[2 * P.N + i.s] = fma(m.jz, inv, P.hgz);
+    rho[i.sl] = m.rho;
+    u[i.sl] = fma(m.jx, inv, P.hgx);
+    u[N + i.sl] = fma(m.jy, inv, P.hgy);
+    u[2 * N + i.sl] = fma(m.jz, inv, P.hgz);
 }
 
 // Pi_ab = sum_i f_i (c_a c_b - delta_ab/3) of the current state (Eq.18 + Eq.19):
@@ -178,19 +187,19 @@ template <typename real, bool WALLS, int MODE>
 __global__ void __launch_bounds__(128)
 stress_kernel(const real* __restrict__ src, real* __restrict__ pi, const FieldParams<real> P)
 {
-    const SiteIndex i = my_site(P.nx, P.ny);
+    const SiteIndex i = my_site(P.G);
     if (!i.valid) return;
     real v[6] = {real(0), real(0), real(0), real(0), real(0), real(0)};
-    if (!(WALLS && (i.z == 0 || i.z == P.nz - 1))) {
+    if (!(WALLS && solid_layer(P.G, i.zg))) {
         real g[3][3][3];
-        gather<real, WALLS, MODE>(src, P.QS, P.nx, P.ny, P.nz, i, g);
+        gather<real, WALLS, MODE>(src, P.G, i, g);
         const Moments10<real> m = forward_moments(g);
         const real third = m.rho * real(1.0 / 3.0);
         v[0] = m.pxx - third; v[1] = m.pyy - third; v[2] = m.pzz - third;
         v[3] = m.pxy; v[4] = m.pxz; v[5] = m.pyz;
     }
 #pragma unroll
-    for (int n = 0; n < 6; ++n) pi[(long long)n * P.N + i.s] = v[n];
+    for (int n = 0; n < 6; ++n) pi[(long long)n * P.G.N + i.sl] = v[n];
 }
 
 // sums over fluid sites of { rho, rho u_x,y,z, u_x,y,z, u_x^2,y^2,z^2 } -> acc[10] (fp64 atomics)
@@ -198,14 +207,14 @@ template <typename real, bool WALLS, int MODE>
 __global__ void __launch_bounds__(128)
 diagnostics_kernel(const real* __restrict__ src, double* __restrict__ acc, const FieldParams<real> P)
 {
-    const SiteIndex i = my_site(P.nx, P.ny);
+    const SiteIndex i = my_site(P.G);
     double v[10];
 #pragma unroll
     for (int n = 0; n < 10; ++n) v[n] = 0.0;
-    const bool fluid = i.valid && !(WALLS && (i.z == 0 || i.z == P.nz - 1));
+    const bool fluid = i.valid && !(WALLS && solid_layer(P.G, i.zg));
     if (fluid) {
         real g[3][3][3];
-        gather<real, WALLS, MODE>(src, P.QS, P.nx, P.ny, P.nz, i, g);
+        gather<real, WALLS, MODE>(src, P.G, i, g);
         const Moments10<real> m = forward_moments(g);
         const double rho = (double)m.rho;
         const double ux = (double)m.jx / rho + (double)P.hgx;
@@ -234,23 +243,32 @@ diagnostics_kernel(const real* __restrict__ src, double* __restrict__ acc, const
 }
 
 // ---------------------------------------------------------------- state import / export (R10)
-// out[canonical i][s] = S_t[i](s): the same gather as the step; solid nodes export their stored values.
+// out[canonical i][sl] = S_t[i](s): the same gather as the step; solid nodes export their stored values.
 template <typename real, bool WALLS, int MODE>
 __global__ void __launch_bounds__(128)
 export_kernel(const real* __restrict__ src, real* __restrict__ out, const FieldParams<real> P)
 {
-    const SiteIndex i = my_site(P.nx, P.ny);
+    const SiteIndex i = my_site(P.G);
     if (!i.valid) return;
-    if (WALLS && (i.z == 0 || i.z == P.nz - 1)) {
+    if (WALLS && solid_layer(P.G, i.zg)) {
 #pragma unroll
-        for (int n = 0; n < Q; ++n) out[(long long)n * P.N + i.s] = src[(long long)lex_of_canon(n) * P.QS + i.s];
+        for (int n = 0; n < Q; ++n) out[(long long)n * P.G.N + i.sl] = src[(long long)lex_of_canon(n) * P.G.QS + i.s];
         return;
     }
     real g[3][3][3];
-    gather<real, WALLS, MODE>(src, P.QS, P.nx, P.ny, P.nz, i, g);
+    gather<real, WALLS, MODE>(src, P.G, i, g);
 #pragma unroll
     for (int n = 0; n < Q; ++n)
-        out[(long long)n * P.N + i.s] = g[canon_cz(n) + 1][canon_cy(n) + 1][canon_cx(n) + 1];
+        out[(long long)n * P.G.N + i.sl] = g[canon_cz(n) + 1][canon_cy(n) + 1][canon_cx(n) + 1];
+}
+
+// index into a canonical INPUT field of the site x + c (periodic in x, y; in z periodic over the nz owned layers, or,
+// in slab mode, plain: the input then has nz + 2 layers, the owned ones at 1..nz)
+__device__ __forceinline__ long long input_index(const Geom& G, int ghost_in, int x, int y, int zl)
+{
+    const int xd = (x + G.nx) % G.nx, yd = (y + G.ny) % G.ny;
+    const int zd = ghost_in ? zl + 1 : (zl + G.nz) % G.nz;
+    return (long long)xd + (long long)G.nx * ((long long)yd + (long long)G.ny * zd);
 }
 
 // P[q](s) = S[q](s + c_q), or S[26-q](s) when s + c_q is solid; solid nodes store S[q](s) unchanged.
@@ -260,28 +278,29 @@ template <typename real, bool WALLS>
 __global__ void __launch_bounds__(128)
 import_kernel(const real* __restrict__ in, real* __restrict__ bufA, real* __restrict__ bufB, const FieldParams<real> P)
 {
-    const SiteIndex i = my_site(P.nx, P.ny);
+    const SiteIndex i = my_site(P.G);
     if (!i.valid) return;
-    const bool solid = WALLS && (i.z == 0 || i.z == P.nz - 1);
+    const Geom& G = P.G;
+    const bool solid = WALLS && solid_layer(G, i.zg);
+    const int zl = (int)blockIdx.z;
+    const long long Nin = (long long)G.nx * G.ny * (G.nz + 2 * P.ghost_in);
 #pragma unroll
     for (int n = 0; n < Q; ++n) {
         const int cx = canon_cx(n), cy = canon_cy(n), cz = canon_cz(n);
         const int q = lex_of(cx, cy, cz);
-        long long from = (long long)n * P.N + i.s;
+        long long from = (long long)n * Nin + input_index(G, P.ghost_in, i.x, i.y, zl);
         if (!solid && !P.aa) {
-            const int zd = i.z + cz;
-            if (WALLS && (zd == 0 || zd == P.nz - 1)) {
+            if (WALLS && solid_layer(G, i.zg + cz)) {
                 // s + c_q solid: this slot is pulled back by the site itself as direction opp(q)
                 const int nopp = canon_of_lex(26 - q);
-                from = (long long)nopp * P.N + i.s;
+                from = (long long)nopp * Nin + input_index(G, P.ghost_in, i.x, i.y, zl);
             } else {
-                const int xd = (i.x + cx + P.nx) % P.nx, yd = (i.y + cy + P.ny) % P.ny, zw = (zd + P.nz) % P.nz;
-                from = (long long)n * P.N + (long long)xd + (long long)P.nx * ((long long)yd + (long long)P.ny * zw);
+                from = (long long)n * Nin + input_index(G, P.ghost_in, i.x + cx, i.y + cy, zl + cz);
             }
         }
         const real v = in[from];
-        bufA[(long long)q * P.QS + i.s] = v;
-        if (bufB != nullptr) bufB[(long long)q * P.QS + i.s] = v;
+        bufA[(long long)q * G.QS + i.s] = v;
+        if (bufB != nullptr) bufB[(long long)q * G.QS + i.s] = v;
     }
 }
 
@@ -302,29 +321,50 @@ __global__ void __launch_bounds__(128)
 init_kernel(const real* __restrict__ rho, const real* __restrict__ u, double rho0, real* __restrict__ bufA,
             real* __restrict__ bufB, const FieldParams<real> P)
 {
-    const SiteIndex i = my_site(P.nx, P.ny);
+    const SiteIndex i = my_site(P.G);
     if (!i.valid) return;
-    const bool solid = WALLS && (i.z == 0 || i.z == P.nz - 1);
+    const Geom& G = P.G;
+    const bool solid = WALLS && solid_layer(G, i.zg);
+    const int zl = (int)blockIdx.z;
+    const long long Nin = (long long)G.nx * G.ny * (G.nz + 2 * P.ghost_in);
 #pragma unroll 1
     for (int q = 0; q < Q; ++q) {
         int cx = q % 3 - 1, cy = (q / 3) % 3 - 1, cz = q / 9 - 1;
-        long long s = i.s;
+        long long s = input_index(G, P.ghost_in, i.x, i.y, zl);
         if (!solid && !P.aa) {
-            const int zd = i.z + cz;
-            if (WALLS && (zd == 0 || zd == P.nz - 1)) {
+            if (WALLS && solid_layer(G, i.zg + cz)) {
                 cx = -cx; cy = -cy; cz = -cz;              // f0 of the opposite direction at the site itself
             } else {
-                const int xd = (i.x + cx + P.nx) % P.nx, yd = (i.y + cy + P.ny) % P.ny, zw = (zd + P.nz) % P.nz;
-                s = (long long)xd + (long long)P.nx * ((long long)yd + (long long)P.ny * zw);
+                s = input_index(G, P.ghost_in, i.x + cx, i.y + cy, zl + cz);
             }
         }
         double r = rho0, ux = 0.0, uy = 0.0, uz = 0.0;
         if (rho != nullptr) {
-            r = (double)rho[s]; ux = (double)u[s]; uy = (double)u[P.N + s]; uz = (double)u[2 * P.N + s];
+            r = (double)rho[s]; ux = (double)u[s]; uy = (double)u[Nin + s]; uz = (double)u[2 * Nin + s];
         }
         const real v = (real)__dmul_rn(__dmul_rn(__dmul_rn(r, phi1d(cx, ux)), phi1d(cy, uy)), phi1d(cz, uz));
-        bufA[(long long)q * P.QS + i.s] = v;
-        if (bufB != nullptr) bufB[(long long)q * P.QS + i.s] = v;
+        bufA[(long long)q * G.QS + i.s] = v;
+        if (bufB != nullptr) bufB[(long long)q * G.QS + i.s] = v;
+    }
+}
+
+// ---------------------------------------------------------------- slab faces (rflbm_halo_pack / rflbm_halo_unpack)
+// One nx x ny face of 9 consecutive storage slots [slot0, slot0 + 9) of storage layer z <-> a packed buffer
+// face[9][ny][nx].  Which layer and which slots depends on scheme and phase (rflbm.cu::halo_plan).
+template <typename real, bool PACK>
+__global__ void __launch_bounds__(128)
+halo_kernel(real* __restrict__ buf, real* __restrict__ face, const Geom G, int z, int slot0)
+{
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
+    if (x >= G.nx || y >= G.ny) return;
+    const long long s = (long long)x + (long long)G.px * y + G.pxy * z;
+    const long long f = (long long)x + (long long)G.nx * y;
+    const long long nf = (long long)G.nx * G.ny;
+#pragma unroll
+    for (int n = 0; n < 9; ++n) {
+        if (PACK) face[n * nf + f] = buf[(long long)(slot0 + n) * G.QS + s];
+        else buf[(long long)(slot0 + n) * G.QS + s] = face[n * nf + f];
     }
 }
 
@@ -339,27 +379,28 @@ debug_rng_kernel(uint32_t* __restrict__ words, real* __restrict__ normals, unsig
     constexpr bool TABLES = sizeof(real) == 8;
     __shared__ f64x2 s_tab[TABLES ? LOG_TABLE_N + SC_TABLE_N : 1];
     if (TABLES) stage_tables(P.tables, s_tab);
-    const SiteIndex i = my_site(P.nx, P.ny);
+    const SiteIndex i = my_site(P.G);
     if (!i.valid) return;
-    const PhiloxSite ps = philox_site((uint32_t)i.s, P.rng);
+    const long long N = P.G.N;
+    const PhiloxSite ps = philox_site(i.site, P.rng);
     bool bad = false;
 #pragma unroll
     for (int call = 0; call < 6; ++call) {
         uint32_t w[4], w_ref[4];
         philox_call(ps, P.rng, call, w);
-        philox4x32_10((uint32_t)i.s, t_hi, t_lo, (uint32_t)call, P.rng, w_ref);
+        philox4x32_10(i.site, t_hi, t_lo, (uint32_t)call, P.rng, w_ref);
         bad = bad || w[0] != w_ref[0] || w[1] != w_ref[1] || w[2] != w_ref[2] || w[3] != w_ref[3];
         if (words != nullptr)
 #pragma unroll
-            for (int mth = 0; mth < 4; ++mth) words[(long long)(4 * call + mth) * P.N + i.s] = w[mth];
+            for (int mth = 0; mth < 4; ++mth) words[(long long)(4 * call + mth) * N + i.sl] = w[mth];
         if (normals != nullptr)
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
                 real z0, z1;
                 normal_pair(w[2 * h], w[2 * h + 1], s_tab, s_tab + LOG_TABLE_N, z0, z1);
                 const int k = 4 + 4 * call + 2 * h;
-                normals[(long long)(k - 4) * P.N + i.s] = z0;
-                if (k + 1 < Q) normals[(long long)(k + 1 - 4) * P.N + i.s] = z1;
+                normals[(long long)(k - 4) * N + i.sl] = z0;
+                if (k + 1 < Q) normals[(long long)(k + 1 - 4) * N + i.sl] = z1;
             }
     }
     if (bad) atomicAdd(mismatch, 1ull);

@@ -29,17 +29,21 @@
 
 namespace rflbm_dev {
 
-constexpr int TILE_X = 128;                   // sites per tile = threads per block
+constexpr int BLOCK_T = 128;                  // threads per block
 constexpr int BOX_Q = 3;                      // populations per box
-constexpr int TMA_MIN_NX = 128;
-// per element type: 16-byte halo on each side of the tile (2 doubles / 4 floats), box = [x0-HALO, x0+128+HALO)
-template <typename real> struct TmaGeom {
+constexpr int TMA_MIN_NX = 32;
+// Tile = TX consecutive x of RB = 128/TX consecutive rows (TX = 128, 64 or 32: every lattice with nx >= 32 takes this
+// kernel).  Per element type: 16-byte halo on each side of a row segment (2 doubles / 4 floats),
+// box = [x0-HALO, x0+TX+HALO) x 3 populations.
+template <typename real, int TX> struct TmaGeom {
     static constexpr int HALO = 16 / (int)sizeof(real);
-    static constexpr int BOX_X = TILE_X + 2 * HALO;                                  // 132 doubles / 136 floats
+    static constexpr int RB = BLOCK_T / TX;                                          // rows per block step
+    static constexpr int BOX_X = TX + 2 * HALO;                                      // 132 doubles / 136 floats at TX = 128
     static constexpr int BOX_BYTES = BOX_X * BOX_Q * (int)sizeof(real);              // 3168 B / 1632 B per copy
     static constexpr int BOX_PITCH_BYTES = (BOX_BYTES + 127) / 128 * 128;            // destinations stay 128-byte aligned
     static constexpr int BOX_PITCH = BOX_PITCH_BYTES / (int)sizeof(real);            // in elements
-    static constexpr int STAGE_BYTES = 9 * BOX_PITCH_BYTES;                          // 28.8 KB / 15.0 KB
+    static constexpr int ROW_STAGE = 9 * BOX_PITCH;                                  // elements per staged row
+    static constexpr int STAGE_BYTES = RB * 9 * BOX_PITCH_BYTES;                     // 28.8 KB / 15.0 KB at TX = 128
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -85,92 +89,107 @@ __device__ __forceinline__ bool elect_one()
     return pred != 0;
 }
 
-// issue the 9 box copies of the tile (x0, y, z); one thread
+// issue the 9 box copies of one row segment (x0, y, z) of the tile; one thread.  The caller has armed the mbarrier.
 // PHASE (rflbm_kernels.cuh): STEP_AB pulls slot q of the neighbour row (bounce-back: slot 26-q of the own row);
 // STEP_AA_EVEN reads slot q of the own row; STEP_AA_ODD pulls slot 26-q of the neighbour row (bounce-back: slot q of
 // the own row).  A box holds three consecutive slots, so "26-q" boxes start at 24-3b-9c and hold the rows reversed.
-template <typename real, bool WALLS, int PHASE>
-__device__ __forceinline__ void issue_tile(const CUtensorMap* tmap, uint32_t s_in, uint32_t bar, int x0, int y, int z,
-                                           int ny, int nz)
+template <typename real, int TX, bool WALLS, int PHASE>
+__device__ __forceinline__ void issue_row(const CUtensorMap* tmap, uint32_t s_in, uint32_t bar, int x0, int y, int z,
+                                          int zg, const Geom& G)
 {
-    using G = TmaGeom<real>;
-    mbar_expect_tx(bar, 9u * (uint32_t)G::BOX_BYTES);
-    const int ys[3] = {(y + 1 == ny) ? 0 : y + 1, y, (y == 0) ? ny - 1 : y - 1};     // y - cy, index b = cy + 1
-    const int zs[3] = {(z + 1 == nz) ? 0 : z + 1, z, (z == 0) ? nz - 1 : z - 1};
+    using T = TmaGeom<real, TX>;
+    const int ys[3] = {(y + 1 == G.ny) ? 0 : y + 1, y, (y == 0) ? G.ny - 1 : y - 1};     // y - cy, index b = cy + 1
+    const int zs[3] = {(z + 1 == G.nzs) ? 0 : z + 1, z, (z == 0) ? G.nzs - 1 : z - 1};   // slab mode: never wraps
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        // with walls the fluid layers are z = 1..nz-2; x - c_q is solid iff (cz=+1 and z==1) or (cz=-1 and z==nz-2):
+        // with walls the fluid layers are zg = 1..nzg-2; x - c_q is solid iff (cz=+1 and zg==1) or (cz=-1 and zg==nzg-2):
         // the population comes back from the site itself as 26-q; the three q' = 26-q of a box are 24-3b-9c + {0,1,2}
-        const bool bounce = WALLS && ((c == 2 && z == 1) || (c == 0 && z == nz - 2));
+        const bool bounce = WALLS && ((c == 2 && zg == 1) || (c == 0 && zg == G.nzg - 2));
 #pragma unroll
         for (int b = 0; b < 3; ++b) {
-            const uint32_t dst = s_in + (uint32_t)((3 * c + b) * G::BOX_PITCH_BYTES);
-            constexpr int fwd = 0, rev = 1;
+            const uint32_t dst = s_in + (uint32_t)((3 * c + b) * T::BOX_PITCH_BYTES);
             const int q_fwd = 3 * b + 9 * c, q_rev = 24 - 3 * b - 9 * c;
-            (void)fwd; (void)rev;
-            if (PHASE == STEP_AA_EVEN) tma_load_box(dst, tmap, x0 - G::HALO, y, z, q_fwd, bar);
-            else if (WALLS && bounce) tma_load_box(dst, tmap, x0 - G::HALO, y, z, PHASE == STEP_AB ? q_rev : q_fwd, bar);
-            else tma_load_box(dst, tmap, x0 - G::HALO, ys[b], zs[c], PHASE == STEP_AB ? q_fwd : q_rev, bar);
+            if (PHASE == STEP_AA_EVEN) tma_load_box(dst, tmap, x0 - T::HALO, y, z, q_fwd, bar);
+            else if (WALLS && bounce) tma_load_box(dst, tmap, x0 - T::HALO, y, z, PHASE == STEP_AB ? q_rev : q_fwd, bar);
+            else tma_load_box(dst, tmap, x0 - T::HALO, ys[b], zs[c], PHASE == STEP_AB ? q_fwd : q_rev, bar);
         }
     }
 }
 
+// the RB rows yb .. yb+RB-1 (those below y_end) of the tile
+template <typename real, int TX, bool WALLS, int PHASE>
+__device__ __forceinline__ void issue_tile(const CUtensorMap* tmap, uint32_t s_in, uint32_t bar, int x0, int yb, int y_end,
+                                           int z, int zg, const Geom& G)
+{
+    using T = TmaGeom<real, TX>;
+    const int nrows = min(T::RB, y_end - yb);
+    mbar_expect_tx(bar, (uint32_t)nrows * 9u * (uint32_t)T::BOX_BYTES);
+#pragma unroll
+    for (int r = 0; r < T::RB; ++r)
+        if (r < nrows)
+            issue_row<real, TX, WALLS, PHASE>(tmap, s_in + (uint32_t)(r * 9 * T::BOX_PITCH_BYTES), bar, x0, yb + r, z, zg, G);
+}
+
 // fp64: 128 registers, 41 KB -> 4 blocks per SM; fp32: 64 registers, 15 KB -> 8 blocks per SM
-template <typename real, bool WALLS, bool FORCE, bool NOISE, bool BGK, bool GHOST, int PHASE>
-__global__ void __launch_bounds__(TILE_X, sizeof(real) == 8 ? 4 : 8)
+template <typename real, int TX, bool WALLS, bool FORCE, bool NOISE, bool BGK, bool GHOST, int PHASE>
+__global__ void __launch_bounds__(BLOCK_T, sizeof(real) == 8 ? 4 : 8)
 step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const real* src, real* dst,
                 const __grid_constant__ StepParams<real> P, int rows)
 {
-    using G = TmaGeom<real>;
+    using T = TmaGeom<real, TX>;
     constexpr bool TABLES = NOISE && sizeof(real) == 8;         // the fp32 Box-Muller needs no tables
-    __shared__ __align__(128) real s_stage[G::STAGE_BYTES / sizeof(real)];
+    __shared__ __align__(128) real s_stage[T::STAGE_BYTES / sizeof(real)];
     __shared__ f64x2 s_tab[TABLES ? LOG_TABLE_N + SC_TABLE_N : 1];
     __shared__ __align__(8) unsigned long long s_bar;
 
-    const int z = blockIdx.z;
-    if (WALLS && (z == 0 || z == P.nz - 1)) return;            // solid layers are never updated
+    const Geom& G = P.G;
+    const int z = (int)blockIdx.z + G.z_lo, zg = z + G.zg0;
+    if (WALLS && solid_layer(G, zg)) return;                   // solid layers are never updated
     const int tid = threadIdx.x;
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);    // warp-uniform for the compiler too
-    const int x0 = blockIdx.x * TILE_X;
+    const int r = (T::RB == 1) ? 0 : __shfl_sync(0xffffffffu, tid / TX, 0);   // row of the tile this warp works on
+    const int xl = tid - r * TX;
+    const int x0 = blockIdx.x * TX;
     const int y_begin = blockIdx.y * rows;
-    const int y_end = min(y_begin + rows, P.ny);
+    const int y_end = min(y_begin + rows, G.ny);
     const uint32_t bar = smem_u32(&s_bar), in0 = smem_u32(&s_stage[0]);
 
     if (warp == 0 && elect_one()) {
         mbar_init(bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        issue_tile<real, WALLS, PHASE>(&tmap_src, in0, bar, x0, y_begin, z, P.ny, P.nz);
+        issue_tile<real, TX, WALLS, PHASE>(&tmap_src, in0, bar, x0, y_begin, y_end, z, zg, G);
     }
     if (TABLES) stage_tables(P.tables, s_tab);                  // ends with __syncthreads()
     else __syncthreads();                                       // mbarrier init visible to every waiter
 
-    const int x = x0 + tid;
-    const bool active = x < P.nx;
-    const bool wrap_lo = (x == 0), wrap_hi = (x == P.nx - 1);
+    const int x = x0 + xl;
+    const bool active = x < G.nx;
+    const bool wrap_lo = (x == 0), wrap_hi = (x == G.nx - 1);
     const bool edge_warp = __any_sync(0xffffffffu, wrap_lo || wrap_hi);
-    const long long nxy = (long long)P.nx * P.ny;
-    const uint32_t QS32 = (uint32_t)P.QS;                        // QS < 2^32 (rflbm_create)
-    const real* tile = &s_stage[0] + tid;
-    const bool bounce_lo = WALLS && z == 1, bounce_hi = WALLS && z == P.nz - 2;
+    const uint32_t QS32 = (uint32_t)G.QS;                        // QS < 2^32 (rflbm_create)
+    const real* tile = &s_stage[0] + r * T::ROW_STAGE + xl;
+    const bool bounce_lo = WALLS && zg == 1, bounce_hi = WALLS && zg == G.nzg - 2;
     uint32_t parity = 0;
 
-    for (int y = y_begin; y < y_end; ++y) {
-        const long long s = (long long)x + (long long)P.nx * y + nxy * z;
+    for (int yb = y_begin; yb < y_end; yb += T::RB) {
+        const int y = yb + r;
+        const bool row_ok = (T::RB == 1) || y < y_end;          // warp-uniform
+        const long long s = (long long)x + (long long)G.px * y + G.pxy * z;
         // periodic wrap in x: TMA zero-fills these 9 values; fetch them early, use them after the barrier
         real wv[3][3];
-        if (PHASE != STEP_AA_EVEN && edge_warp) {               // warp-uniform branch: interior warps skip all of this
+        if (PHASE != STEP_AA_EVEN && edge_warp && row_ok) {     // warp-uniform branch: interior warps skip all of this
             if (wrap_lo || wrap_hi) {
-                const int ysr[3] = {(y + 1 == P.ny) ? 0 : y + 1, y, (y == 0) ? P.ny - 1 : y - 1};
-                const int zsr[3] = {(z + 1 == P.nz) ? 0 : z + 1, z, (z == 0) ? P.nz - 1 : z - 1};
+                const int ysr[3] = {(y + 1 == G.ny) ? 0 : y + 1, y, (y == 0) ? G.ny - 1 : y - 1};
+                const int zsr[3] = {(z + 1 == G.nzs) ? 0 : z + 1, z, (z == 0) ? G.nzs - 1 : z - 1};
 #pragma unroll
                 for (int c = 0; c < 3; ++c)
 #pragma unroll
                     for (int b = 0; b < 3; ++b) {
-                        const long long row = (long long)P.nx * ysr[b] + nxy * zsr[c];
-                        // x+1 -> 0 for cx = -1 (a = 0); x-1 -> nx-1 for cx = +1 (a = 2); nx >= 128 here
+                        const long long row = (long long)G.px * ysr[b] + G.pxy * zsr[c];
+                        // x+1 -> 0 for cx = -1 (a = 0); x-1 -> nx-1 for cx = +1 (a = 2); nx >= 32 here
                         const int qa = (wrap_hi ? 0 : 2) + 3 * b + 9 * c;
                         const int slot = (PHASE == STEP_AB) ? qa : 26 - qa;
-                        const long long at = (long long)slot * P.QS + row + (wrap_hi ? 0 : P.nx - 1);
+                        const long long at = (long long)slot * G.QS + row + (wrap_hi ? 0 : G.nx - 1);
                         wv[c][b] = (PHASE == STEP_AB) ? __ldg(src + at) : src[at];   // AA: the buffer is written in place
                     }
             }
@@ -183,34 +202,35 @@ step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const real* src, r
             const bool bounce = (c == 2 && bounce_lo) || (c == 0 && bounce_hi);
 #pragma unroll
             for (int b = 0; b < 3; ++b) {
-                const real* box = tile + (3 * c + b) * G::BOX_PITCH;
+                const real* box = tile + (3 * c + b) * T::BOX_PITCH;
                 // forward boxes hold slots q in rows a = 0,1,2; reversed boxes hold q' = 26-q in ascending q': row 2-a.
-                // Pulled rows are read with the x shift -cx, local ones (bounce-back, even AA phase) at tid+HALO.
+                // Pulled rows are read with the x shift -cx, local ones (bounce-back, even AA phase) at xl+HALO.
                 const bool local = (PHASE == STEP_AA_EVEN) || (WALLS && bounce);
                 const bool reversed = (PHASE == STEP_AB) ? (WALLS && bounce) : (PHASE == STEP_AA_ODD && !(WALLS && bounce));
                 if (local && reversed) {
-                    g[c][b][0] = box[2 * G::BOX_X + G::HALO];
-                    g[c][b][1] = box[1 * G::BOX_X + G::HALO];
-                    g[c][b][2] = box[0 * G::BOX_X + G::HALO];
+                    g[c][b][0] = box[2 * T::BOX_X + T::HALO];
+                    g[c][b][1] = box[1 * T::BOX_X + T::HALO];
+                    g[c][b][2] = box[0 * T::BOX_X + T::HALO];
                 } else if (local) {
-                    g[c][b][0] = box[0 * G::BOX_X + G::HALO];
-                    g[c][b][1] = box[1 * G::BOX_X + G::HALO];
-                    g[c][b][2] = box[2 * G::BOX_X + G::HALO];
+                    g[c][b][0] = box[0 * T::BOX_X + T::HALO];
+                    g[c][b][1] = box[1 * T::BOX_X + T::HALO];
+                    g[c][b][2] = box[2 * T::BOX_X + T::HALO];
                 } else if (reversed) {
-                    g[c][b][0] = box[2 * G::BOX_X + G::HALO + 1];
-                    g[c][b][1] = box[1 * G::BOX_X + G::HALO];
-                    g[c][b][2] = box[0 * G::BOX_X + G::HALO - 1];
+                    g[c][b][0] = box[2 * T::BOX_X + T::HALO + 1];
+                    g[c][b][1] = box[1 * T::BOX_X + T::HALO];
+                    g[c][b][2] = box[0 * T::BOX_X + T::HALO - 1];
                 } else {
-                    g[c][b][0] = box[0 * G::BOX_X + G::HALO + 1];
-                    g[c][b][1] = box[1 * G::BOX_X + G::HALO];
-                    g[c][b][2] = box[2 * G::BOX_X + G::HALO - 1];
+                    g[c][b][0] = box[0 * T::BOX_X + T::HALO + 1];
+                    g[c][b][1] = box[1 * T::BOX_X + T::HALO];
+                    g[c][b][2] = box[2 * T::BOX_X + T::HALO - 1];
                 }
             }
         }
         __syncthreads();                                       // the tile is in registers: the stage is free
-        if (warp == 0 && y + 1 < y_end && elect_one()) issue_tile<real, WALLS, PHASE>(&tmap_src, in0, bar, x0, y + 1, z, P.ny, P.nz);
+        if (warp == 0 && yb + T::RB < y_end && elect_one())
+            issue_tile<real, TX, WALLS, PHASE>(&tmap_src, in0, bar, x0, yb + T::RB, y_end, z, zg, G);
 
-        if (PHASE != STEP_AA_EVEN && edge_warp) {
+        if (PHASE != STEP_AA_EVEN && edge_warp && row_ok) {
             if (wrap_lo || wrap_hi) {
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
@@ -224,14 +244,15 @@ step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const real* src, r
                 }
             }
         }
-        if (active) {
-            collide<real, FORCE, NOISE, BGK, GHOST>(g, P, (uint32_t)s, s_tab, s_tab + LOG_TABLE_N);
+        if (active && row_ok) {
+            const uint32_t site = (uint32_t)((long long)x + (long long)G.nx * ((long long)y + (long long)G.ny * (long long)zg));
+            collide<real, FORCE, NOISE, BGK, GHOST>(g, P, site, s_tab, s_tab + LOG_TABLE_N);
             if (PHASE == STEP_AA_ODD) {
                 // push to the neighbours x + c_q (slot q), misaligned by one element for cx = +-1: the partial
                 // sectors at the ends of a warp's 256 bytes are completed in L2 by the neighbouring warp's store
                 SiteIndex i;
-                i.x = x; i.y = y; i.z = z; i.valid = true; i.s = s;
-                scatter<real, WALLS, STEP_AA_ODD>(dst, P.QS, P.nx, P.ny, P.nz, i, g);
+                i.x = x; i.y = y; i.z = z; i.zg = zg; i.valid = true; i.s = s; i.sl = 0; i.site = site;
+                scatter<real, WALLS, STEP_AA_ODD>(dst, G, i, g);
             } else {
                 const unsigned long long out = reinterpret_cast<unsigned long long>(dst + s);
 #pragma unroll

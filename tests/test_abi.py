@@ -64,6 +64,52 @@ def test_create_validation_and_workspace_size(lib):
     lib.rflbm_destroy(h32)
 
 
+def test_slab_and_grid_validation_host_side(lib):
+    """rflbm_set_slab / halo argument checks and the launch-grid limits of rflbm_create: host only, no GPU work."""
+    h = C.c_void_p()
+    # padded row pitch: nx = 33 fp64 rows are 48 elements (whole 128-byte lines), slab adds two ghost layers
+    assert lib.rflbm_create(33, 4, 5, 1.0, 1e-4, 1.0, 0, binding.F64, C.byref(h)) == binding.OK
+    plain = lib.rflbm_workspace_bytes(h)
+    assert plain == 2 * 27 * (48 * 4 * 5) * 8 + 4096 + 12288
+    assert lib.rflbm_halo_bytes(h) == 9 * 33 * 4 * 8
+    assert lib.rflbm_halo_pending(h) == 0
+    assert lib.rflbm_halo_pack(h, binding.SIDE_LOW, 0x1000) == binding.ESTATE          # not in slab mode
+    assert lib.rflbm_set_slab(h, -1, 20) == binding.EINVAL
+    assert lib.rflbm_set_slab(h, 16, 20) == binding.EINVAL                                # [16, 21) does not fit
+    assert lib.rflbm_set_slab(h, 0, 1 << 30) == binding.EINVAL                            # 2^32 global sites or more
+    assert lib.rflbm_workspace_bytes(h) == plain                                          # failed calls change nothing
+    assert lib.rflbm_set_slab(h, 15, 20) == binding.OK
+    assert lib.rflbm_workspace_bytes(h) == 2 * 27 * (48 * 4 * 7) * 8 + 4096 + 12288
+    assert lib.rflbm_halo_pack(h, binding.SIDE_LOW, 0x1000) == binding.ESTATE          # before init
+    assert lib.rflbm_halo_pack(h, 2, 0x1000) == binding.EINVAL
+    assert lib.rflbm_halo_unpack(h, binding.SIDE_HIGH, None) == binding.EINVAL
+    assert lib.rflbm_set_walls_z(h, 1) == binding.OK                                      # walls look at nz_global = 20
+    assert lib.rflbm_last_kernel(h) == b""
+    lib.rflbm_destroy(h)
+    assert lib.rflbm_create(4, 4, 2, 1.0, 0.0, 1.0, 0, binding.F64, C.byref(h)) == binding.OK
+    assert lib.rflbm_set_walls_z(h, 1) == binding.EINVAL                                  # nz = 2
+    assert lib.rflbm_set_slab(h, 3, 8) == binding.OK
+    assert lib.rflbm_set_walls_z(h, 1) == binding.OK                                      # nz_global = 8
+    lib.rflbm_destroy(h)
+    # gridDim.y <= 65535 blocks: nx >= 128 -> one row per block row; nx = 8 -> 16 rows per block
+    assert lib.rflbm_create(128, 70000, 1, 1.0, 0.0, 1.0, 0, binding.F64, C.byref(h)) == binding.EINVAL
+    assert lib.rflbm_create(128, 65535, 1, 1.0, 0.0, 1.0, 0, binding.F64, C.byref(h)) == binding.OK
+    lib.rflbm_destroy(h)
+    assert lib.rflbm_create(8, 70000, 1, 1.0, 0.0, 1.0, 0, binding.F64, C.byref(h)) == binding.OK
+    lib.rflbm_destroy(h)
+    assert lib.rflbm_create(1, 1, 70000, 1.0, 0.0, 1.0, 0, binding.F64, C.byref(h)) == binding.EINVAL
+
+
+def test_no_environment_knobs_in_the_product():
+    """the C-ABI's layout and launch shape must not depend on the caller's environment"""
+    pkg = os.path.join(ROOT, "paper_2507_08820_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".cu", ".cuh", ".h", ".py")) and f != "build.py":
+                s = open(os.path.join(dirpath, f)).read()
+                assert "getenv" not in s and "os.environ" not in s, f
+
+
 def test_binding_fails_loudly_without_cuda():
     import torch
     if torch.cuda.is_available():

@@ -124,14 +124,22 @@ def test_fp32_channel_parity_100_steps():
     w_g, n_g = sim.debug_rng(17)
     w_r, n_r = ref.debug_rng(17)
     assert np.array_equal(w_g.cpu().numpy().view(np.uint32), w_r)
-    assert np.abs(n_g.cpu().numpy().astype(np.float64) - n_r).max() < 5e-4     # float Box-Muller, |r| up to 5.9
+    nerr = np.abs(n_g.cpu().numpy().astype(np.float64) - n_r).max()
+    # R14: the fp32 Box-Muller runs on the special-function unit; DESIGN.md states 1e-5 on a normal (derived bound
+    # 4e-6: lg2.approx 2^-22 absolute at the radius R = 0.044 where the series takes over, sin/cos.approx 2^-21.4
+    # times |R| <= 5.9; measured 1.8e-6 over 5.6e6 draws).  A population sees sqrt(3 kT rho) w_i/b_k times that.
+    print(f"fp32 parity after 100 steps: max|f_gpu - f_oracle| = {err:.3e} (tolerance {TOL32:g}); "
+          f"max|normal_gpu - normal_oracle| = {nerr:.3e} (tolerance 1e-5)")
+    assert nerr < 1e-5, nerr
 
 
 def test_fp32_periodic_parity():
     sim, ref = make_pair(20, 12, 7, 0.7, 1e-4, 8, precision=binding.F32)
     init_pair(sim, ref, synthetic.smooth_random_fields(20, 12, 7, 2))
     sim.step(100); ref.step(100)
-    assert np.abs(pops(sim) - ref.get_populations()).max() < TOL32
+    err = np.abs(pops(sim) - ref.get_populations()).max()
+    print(f"fp32 periodic parity after 100 steps: max|f_gpu - f_oracle| = {err:.3e} (tolerance {TOL32:g})")
+    assert err < TOL32, err
 
 
 def test_set_get_roundtrip_and_resume_bit_exact():
@@ -193,10 +201,15 @@ def test_run_host_matches_device_path():
 
 @pytest.mark.parametrize("shape,walls,force,kT", [((128, 4, 3), False, None, 1e-4), ((256, 5, 4), True, (1e-5, 2e-6, -3e-6), 1e-4),
                                                  ((300, 3, 3), False, None, 1e-4), ((130, 18, 5), True, None, 0.0),
-                                                 ((384, 20, 2), False, (1e-6, 0.0, 0.0), 1e-3)])
+                                                 ((384, 20, 2), False, (1e-6, 0.0, 0.0), 1e-3),
+                                                 ((129, 7, 5), False, None, 1e-4), ((131, 19, 4), True, (1e-5, 0.0, 0.0), 1e-4),
+                                                 ((32, 9, 4), False, None, 1e-4), ((33, 35, 3), True, None, 1e-4),
+                                                 ((64, 17, 3), False, (1e-6, 1e-6, 0.0), 1e-4), ((100, 6, 5), True, None, 1e-4),
+                                                 ((127, 33, 2), False, None, 1e-4)])
 def test_tma_kernel_matches_plain_kernel_and_oracle(shape, walls, force, kT):
-    """The TMA-staged step kernel (fp64, nx >= 128, nx even) against the plain kernel (bit for bit: same
-    arithmetic) and the oracle; shapes span several x tiles, a ragged last tile, > rows_per_block rows, walls."""
+    """The TMA-staged step kernel (fp64; tiles of 128, 64 or 32 sites; any nx >= 32, odd ones included: the internal
+    row pitch is padded) against the plain kernel (bit for bit: same arithmetic) and the oracle; shapes span several
+    x tiles, a ragged last tile, > rows_per_block rows, ragged row groups of the narrow tiles, walls."""
     torch = torch_()
     nx, ny, nz = shape
     fields = synthetic.smooth_random_fields(nx, ny, nz, 13)
@@ -213,9 +226,11 @@ def test_tma_kernel_matches_plain_kernel_and_oracle(shape, walls, force, kT):
 
 
 @pytest.mark.parametrize("shape,walls,force,kT", [((128, 5, 4), False, None, 1e-4), ((260, 18, 5), True, (1e-5, 2e-6, -3e-6), 1e-4),
-                                                 ((384, 3, 3), False, (1e-6, 0.0, 0.0), 0.0)])
+                                                 ((384, 3, 3), False, (1e-6, 0.0, 0.0), 0.0), ((130, 7, 5), False, None, 1e-4),
+                                                 ((131, 6, 4), True, None, 1e-4), ((33, 19, 3), False, None, 1e-4),
+                                                 ((66, 9, 5), True, (1e-6, 0.0, 0.0), 1e-4)])
 def test_tma_kernel_fp32_matches_plain_kernel_and_oracle(shape, walls, force, kT):
-    """fp32 instantiation of the TMA kernel (nx >= 128, nx % 4 == 0): 136-float boxes, 4-element halo."""
+    """fp32 instantiation of the TMA kernel (any nx >= 32): 136-float boxes at TX = 128, 4-element halo."""
     torch = torch_()
     nx, ny, nz = shape
     fields = synthetic.smooth_random_fields(nx, ny, nz, 14)
@@ -231,20 +246,27 @@ def test_tma_kernel_fp32_matches_plain_kernel_and_oracle(shape, walls, force, kT
     assert np.abs(outs[binding.KERNEL_TMA].cpu().numpy().astype(np.float64) - ref.get_populations()).max() < TOL32
 
 
-def test_tma_variant_rejected_when_lattice_does_not_allow_it():
-    for nx, prec in ((33, binding.F64), (130, binding.F32)):     # too short; row pitch 520 B not a multiple of 16
+def test_tma_variant_rejected_only_below_32_and_auto_never_takes_the_plain_kernel_with_noise():
+    for nx, prec in ((31, binding.F64), (8, binding.F32)):       # shorter than the narrowest tile
         sim = binding.Rflbm(nx, 4, 4, 0.8, 1e-4, precision=prec)
         sim.set_kernel_variant(binding.KERNEL_TMA)
         sim.init()
         with pytest.raises(binding.RflbmError) as e:
             sim.step(1)
         assert e.value.code == binding.EINVAL
-    sim = binding.Rflbm(33, 4, 4, 0.8, 1e-4)
-    sim.set_kernel_variant(binding.KERNEL_TMA)
-    sim.init()
-    with pytest.raises(binding.RflbmError) as e:
-        sim.step(1)
-    assert e.value.code == binding.EINVAL
+    # AUTO with noise: every lattice with nx >= 32 runs the TMA kernel (the internal row pitch is padded, so odd nx
+    # qualifies); kT = 0 keeps the plain kernel (pure streaming, where it is the faster one)
+    for nx, prec, name in ((32, binding.F64, "TX=32"), (33, binding.F32, "TX=32"), (64, binding.F64, "TX=64"),
+                           (127, binding.F32, "TX=64"), (129, binding.F64, "TX=128"), (130, binding.F32, "TX=128"),
+                           (511, binding.F64, "TX=128")):
+        sim = binding.Rflbm(nx, 3, 3, 0.8, 1e-4, precision=prec)
+        assert sim.last_kernel == ""
+        sim.init(); sim.step(2)
+        assert sim.last_kernel == f"step_kernel_tma<{name}>", (nx, sim.last_kernel)
+    sim = binding.Rflbm(16, 3, 3, 0.8, 1e-4); sim.init(); sim.step(1)
+    assert sim.last_kernel == "step_kernel"
+    sim = binding.Rflbm(256, 3, 3, 0.8, 0.0); sim.init(); sim.step(1)
+    assert sim.last_kernel == "step_kernel"
 
 
 @pytest.mark.parametrize("shape,prec,walls,kT,tau", [((16, 16, 16), binding.F64, False, 1e-4, 1.0), ((5, 7, 9), binding.F64, False, 1e-4, 0.55),
@@ -257,7 +279,7 @@ def test_bgk_flbm_model_matches_oracle(shape, prec, walls, kT, tau):
     nx, ny, nz = shape
     fields = synthetic.smooth_random_fields(nx, ny, nz, 23)
     outs = []
-    variants = [binding.KERNEL_PLAIN] + ([binding.KERNEL_TMA] if nx >= 128 else [])
+    variants = [binding.KERNEL_PLAIN] + ([binding.KERNEL_TMA] if nx >= 32 else [])
     for variant in variants:
         sim, ref = make_pair(nx, ny, nz, tau, kT, 29, precision=prec, walls=walls)
         sim.set_model(binding.MODEL_BGK); ref.set_model(oracle.MODEL_BGK)
