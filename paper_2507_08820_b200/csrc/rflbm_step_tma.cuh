@@ -56,6 +56,10 @@ __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 {
     uint32_t ok, spins = 0;
@@ -141,6 +145,9 @@ step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const real* src, r
     __shared__ __align__(128) real s_stage[T::STAGE_BYTES / sizeof(real)];
     __shared__ f64x2 s_tab[TABLES ? LOG_TABLE_N + SC_TABLE_N : 1];
     __shared__ __align__(8) unsigned long long s_bar;
+#ifdef RFLBM_EXP_NOSYNC
+    __shared__ __align__(8) unsigned long long s_empty;      // consumer release: one arrival per warp
+#endif
 
     const Geom& G = P.G;
     const int z = (int)blockIdx.z + G.z_lo, zg = z + G.zg0;
@@ -154,8 +161,14 @@ step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const real* src, r
     const int y_end = min(y_begin + rows, G.ny);
     const uint32_t bar = smem_u32(&s_bar), in0 = smem_u32(&s_stage[0]);
 
+#ifdef RFLBM_EXP_NOSYNC
+    const uint32_t empty = smem_u32(&s_empty);
+#endif
     if (warp == 0 && elect_one()) {
         mbar_init(bar, 1);
+#ifdef RFLBM_EXP_NOSYNC
+        mbar_init(empty, BLOCK_T / 32);
+#endif
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         issue_tile<real, TX, WALLS, PHASE>(&tmap_src, in0, bar, x0, y_begin, y_end, z, zg, G);
     }
@@ -226,9 +239,19 @@ step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const real* src, r
                 }
             }
         }
+#ifdef RFLBM_EXP_NOSYNC
+        // the tile is in registers: every warp releases the stage; only the issuing lane waits for all four
+        __syncwarp();
+        if (elect_one()) mbar_arrive(empty);
+        if (warp == 0 && yb + T::RB < y_end && elect_one()) {
+            mbar_wait(empty, parity ^ 1u);
+            issue_tile<real, TX, WALLS, PHASE>(&tmap_src, in0, bar, x0, yb + T::RB, y_end, z, zg, G);
+        }
+#else
         __syncthreads();                                       // the tile is in registers: the stage is free
         if (warp == 0 && yb + T::RB < y_end && elect_one())
             issue_tile<real, TX, WALLS, PHASE>(&tmap_src, in0, bar, x0, yb + T::RB, y_end, z, zg, G);
+#endif
 
         if (PHASE != STEP_AA_EVEN && edge_warp && row_ok) {
             if (wrap_lo || wrap_hi) {

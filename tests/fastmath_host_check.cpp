@@ -1,4 +1,5 @@
-// fastmath_host_check.cpp — host build of rflbm_fastmath.cuh for tests/test_fastmath_host.py (CPU only).
+// fastmath_host_check.cpp — TEST SHIM: host build of csrc/rflbm_fastmath.cuh for tests/test_fastmath_host.py (CPU
+// only; compiled by that test with -I paper_2507_08820_b200/csrc).
 // Exposes the CUDA path's own Box-Muller pieces (compiled for the host) so that they can be compared with
 // long-double libm over the whole 32-bit input range.  Not part of librflbm.so; shares nothing with oracle/.
 #include "rflbm_fastmath.cuh"

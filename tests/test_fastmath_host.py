@@ -1,5 +1,5 @@
-"""CPU check of the CUDA path's own Box-Muller routines (csrc/rflbm_fastmath.cuh compiled for the host through
-csrc/fastmath_host_check.cpp) against 80-bit long-double libm over the whole 32-bit input range.
+"""CPU check of the CUDA path's own Box-Muller routines (csrc/rflbm_fastmath.cuh compiled for the host through the
+test shim tests/fastmath_host_check.cpp) against 80-bit long-double libm over the whole 32-bit input range.
 
 This is host logic of the product, not the oracle: nothing under oracle/ is used here.  The device differs from
 this host build only in the reciprocal-square-root seed (MUFU.RSQ64H vs a truncated 1/sqrt), which the third-order
@@ -12,7 +12,8 @@ import numpy as np
 import pytest
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-SRC = os.path.join(ROOT, "paper_2507_08820_b200", "csrc", "fastmath_host_check.cpp")
+SRC = os.path.join(ROOT, "tests", "fastmath_host_check.cpp")
+INC = os.path.join(ROOT, "paper_2507_08820_b200", "csrc")
 LD = np.longdouble
 pytestmark = pytest.mark.skipif(np.finfo(LD).nmant < 63, reason="needs 80-bit long double")
 
@@ -20,7 +21,7 @@ pytestmark = pytest.mark.skipif(np.finfo(LD).nmant < 63, reason="needs 80-bit lo
 @pytest.fixture(scope="module")
 def fm(tmp_path_factory):
     so = str(tmp_path_factory.mktemp("fm") / "libfm.so")
-    subprocess.run(["g++", "-O2", "-std=c++17", "-ffp-contract=off", "-shared", "-fPIC", "-o", so, SRC], check=True)
+    subprocess.run(["g++", "-O2", "-std=c++17", "-ffp-contract=off", "-shared", "-fPIC", "-I", INC, "-o", so, SRC], check=True)
     return C.CDLL(so)
 
 
