@@ -134,24 +134,24 @@ __device__ __forceinline__ void normal_polar(uint32_t xa, uint32_t xb, const f64
 // sincospif cost ~45 instructions per pair and halved the throughput, profiles/r01d):
 //   -2 ln u = (-2 ln 2) lg2.approx(u)   (MUFU.LG2, abs. error < 2^-22 on lg2, u in [2^-25, 1))
 //   (for u within 2^-10 of 1 the series 2v + v^2 of -2 ln(1-v), v = 1-u exact, replaces it: R error < 1e-5 everywhere)
-//   R = W rsqrt.approx(W)                (MUFU.RSQ, 2 ulp; W >= 5.9e-8 > 0)
+//   R = sqrt.approx(W)                   (MUFU.SQRT, 2^-23 relative; W >= 5.9e-8 > 0)
 //   sin, cos(2 pi u) = -sin, -cos(2 pi u - pi), argument in (-pi, pi) where MUFU.SIN/COS are good to 2^-21.4
 __device__ __forceinline__ void normal_polar(uint32_t xa, uint32_t xb, const f64x2*, const f64x2*, float& R, float& sn,
                                              float& cs)
 {
     const uint32_t k = xa >> 8;
-    const float ua = ((float)k + 0.5f) * (1.0f / 16777216.0f);     // rounds to 1.0f for the last k: handled below
-    float l2, rs;
+    const float ua = fmaf((float)k, 1.0f / 16777216.0f, 1.0f / 33554432.0f);   // (k + 1/2)/2^24, one rounding; 1.0f for the last k: handled below
+    float l2;
     asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(l2) : "f"(ua));        // ua is a normal number: no denormal scaling needed
     float W = -1.3862943611198906f * l2;
     if (k >= 16777216u - 16384u) {                                  // u within 2^-10 of 1 (3 % of the warps): the
         const float v = ((float)(16777216u - k) - 0.5f) * (1.0f / 16777216.0f);   // absolute error of lg2 would show,
         W = fmaf(v, v, 2.0f * v);                                   // so -2 ln(1-v) = 2v + v^2 + O(v^3 < 1e-9), v exact
     }
-    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(rs) : "f"(W));
-    R = W * rs;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(R) : "f"(W));         // MUFU.SQRT, relative error 2^-23; W >= 5.9e-8 > 0
     // 2 pi u - pi = 2 pi ((xb>>8) - 2^23 + 0.5) / 2^24, exact integer part
-    const float th = ((float)((int)(xb >> 8) - 8388608) + 0.5f) * (6.283185307179586f / 16777216.0f);
+    constexpr float TWO_PI_24 = 6.283185307179586f / 16777216.0f;
+    const float th = fmaf((float)((int)(xb >> 8) - 8388608), TWO_PI_24, 0.5f * TWO_PI_24);
     float s, c;
     __sincosf(th, &s, &c);
     sn = -s;

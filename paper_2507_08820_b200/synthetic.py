@@ -63,3 +63,13 @@ def random_population_field(nx, ny, nz, seed, scale, spread=0.02):
     rng = np.random.default_rng(seed)
     scale = np.asarray(scale, np.float64).reshape(27, 1, 1, 1)
     return scale * (1.0 + spread * rng.uniform(-1.0, 1.0, size=(27, nz, ny, nx)))
+
+
+def gaussian_population_field(nx, ny, nz, seed, mean, std):
+    """Independent Gaussian populations f[27,nz,ny,nx] = mean[i] + std[i] * N(0,1); `mean` and `std` (27 values each)
+    are supplied by the caller (e.g. lattice weights and the thermal standard deviation of whichever implementation
+    is under test): no lattice or physics constant lives here."""
+    rng = np.random.default_rng(seed)
+    mean = np.asarray(mean, np.float64).reshape(27, 1, 1, 1)
+    std = np.asarray(std, np.float64).reshape(27, 1, 1, 1)
+    return mean + std * rng.standard_normal(size=(27, nz, ny, nx))

@@ -179,22 +179,12 @@ def test_config5_channel_fp32_startup_profile_256():
     assert abs(d1[0] / d0[0] - 1.0) < 1e-5                           # fp32 storage: mass drift reported and bounded
 
 
-@pytest.mark.parametrize("model,tau", [("reg", 0.51), ("reg", 1.0), ("reg", 50.0), ("bgk", 1.0), ("bgk", 50.0)])
-def test_table_III_trend_equilibration_ratios_64(model, tau):
-    """Reduced-scale Table III (64^3 and 2e4 steps instead of 256^3 and 5e5, kT = 1/3000 as in
-    :254): ER of rho, momentum, diagonal and off-diagonal Hermite stress = variance / (rho0 kT b_k / cs2).
-    Reg-FLBM: within 0.5 % of 1 for 0.51 <= tau <= 100 (:260), reproduced here.
-    BGK-FLBM with reading R19 (all 23 modes thermalised at the one omega) ALSO equilibrates to 1.000 at tau = 50;
-    the paper's BGK column (0.953 / 0.930 at tau >= 50) is not reproduced by Eq.11 as printed — DESIGN.md section 10."""
+def _equilibration_ratios(sim, c, kT, until, every):
+    """ER of rho, momentum, diagonal and off-diagonal Hermite stress over the lattice:
+    variance / (rho0 kT b_k / cs2), averaged over snapshots taken `every` steps apart."""
     torch = torch_()
-    n, kT = 64, 1.0 / 3000.0
-    c = torch.tensor(oracle.tables()[0], dtype=torch.float64, device="cuda")
-    sim = binding.Rflbm(n, n, n, tau, kT, 1.0, 9)
-    sim.set_model(binding.MODEL_BGK if model == "bgk" else binding.MODEL_REG)
-    sim.init()
-    sim.step(4000)
     er = []
-    while sim.step_count <= 20000:
+    while sim.step_count <= until:
         f = sim.get_populations().reshape(27, -1)
         rho = f.sum(0)
         j = c.T @ f
@@ -203,12 +193,71 @@ def test_table_III_trend_equilibration_ratios_64(model, tau):
         er.append([float(rho.var(unbiased=False)) / (3 * kT), float(j.var(dim=1, unbiased=False).mean()) / kT,
                    float(pd.var(dim=1, unbiased=False).mean()) / (2.0 / 3.0 * kT),
                    float(po.var(dim=1, unbiased=False).mean()) / (1.0 / 3.0 * kT)])
-        sim.step(200)
-    er = np.mean(er, axis=0)
-    print(model, tau, "ER(rho, j, Pi_aa, Pi_ab) =", np.round(er, 4))
-    # tau = 0.51 sits at the edge of the paper's 0.5 % band: Table III prints 1.005 / 1.013 / 1.004 / 1.012 there
-    # (measured here: 1.003 / 1.006 / 1.006 / 1.005)
-    assert np.abs(er - 1.0).max() < (0.015 if tau < 0.55 else 0.005), er
+        sim.step(every)
+    return np.mean(er, axis=0)
+
+
+def _thermal_populations(n, kT, seed):
+    """independent Gaussian populations of variance 3 kT rho0 w_i around w_i: the equilibrium measure of the
+    fluctuating model (P8), so that the slow hydrodynamic modes of a tau -> 1/2 run start thermalised"""
+    torch = torch_()
+    w = torch.tensor(oracle.tables()[1], dtype=torch.float64, device="cuda").reshape(27, 1, 1, 1)
+    gen = torch.Generator(device="cuda").manual_seed(seed)
+    return w + torch.sqrt(3.0 * kT * w) * torch.randn((27, n, n, n), dtype=torch.float64, device="cuda", generator=gen)
+
+
+def test_table_III_reduced_sweep_regflbm_all_14_tau(golden_dir):
+    """Reduced Table III: all 14 relaxation times of the Reg-FLBM column at 64^3 and 2e4 steps
+    instead of 256^3 and 5e5, kT = 1/3000 (:254), from a thermal start, printed beside the paper's row
+    (tests/golden/table_III_regflbm.txt).  Gated: only what the paper states in words -
+      * "within 0.5 %" of 1 for 0.51 <~ tau <~ 100 (:260): |ER - 1| < 0.005 for 0.55 <= tau <= 100, and < 0.016 at
+        tau = 0.505 and 0.51, where Table III itself prints up to 1.016;
+      * stable down to tau = 0.5001 with the errors GROWING as tau -> 1/2 (:268), and of the printed sign (ER > 1).
+    The distance to the printed values is reported and bracketed at 0.03 (this build's bracket: the lattice is 64
+    times smaller and the run 25 times shorter than the paper's)."""
+    torch = torch_()
+    n, kT = 64, 1.0 / 3000.0
+    c = torch.tensor(oracle.tables()[0], dtype=torch.float64, device="cuda")
+    rows = [[float(v) for v in ln.split()] for ln in open(golden_dir + "/table_III_regflbm.txt")
+            if ln.strip() and not ln.startswith("#")]
+    assert len(rows) == 14
+    got = {}
+    print("\n   tau    ER(rho, j, Pi_aa, Pi_ab) here (64^3, 2e4 steps)   |  Table III (256^3, 5e5 steps)")
+    for tau, *paper in rows:
+        sim = binding.Rflbm(n, n, n, tau, kT, 1.0, 9)
+        sim.set_populations(_thermal_populations(n, kT, 99), 0)
+        sim.step(2000)
+        er = _equilibration_ratios(sim, c, kT, 20000, 200)
+        got[tau] = er
+        print(f"{tau:8.4f}  " + "  ".join(f"{v:6.4f}" for v in er) + "   |  " + "  ".join(f"{v:5.3f}" for v in paper))
+        assert np.isfinite(er).all(), tau                                   # stable (:268)
+        assert np.abs(er - np.array(paper)).max() < 0.03, (tau, er, paper)  # reported distance, this build's bracket
+        if tau >= 0.55:
+            assert np.abs(er - 1.0).max() < 0.005, (tau, er)                # :260
+        elif tau >= 0.505:
+            assert np.abs(er - 1.0).max() < 0.016, (tau, er)
+        else:
+            assert (er > 1.005).all(), (tau, er)                            # the printed sign of the excess
+    # errors grow as tau -> 1/2 (:268): momentum and both stress ratios are ordered like the printed column
+    for k in (1, 2, 3):
+        col = [got[t][k] for t in (0.5001, 0.5005, 0.501, 0.505, 0.51, 0.55)]
+        assert all(a > b for a, b in zip(col, col[1:])), (k, col)
+
+
+@pytest.mark.parametrize("tau", [1.0, 50.0])
+def test_table_III_bgk_flbm_reading_R19_64(tau):
+    """BGK-FLBM with reading R19 (all 23 modes thermalised at the one omega) ALSO equilibrates to 1.000 at tau = 50;
+    the paper's BGK column (0.953 / 0.930 at tau >= 50) is not reproduced by Eq.11 as printed — DESIGN.md section 10."""
+    torch = torch_()
+    n, kT = 64, 1.0 / 3000.0
+    c = torch.tensor(oracle.tables()[0], dtype=torch.float64, device="cuda")
+    sim = binding.Rflbm(n, n, n, tau, kT, 1.0, 9)
+    sim.set_model(binding.MODEL_BGK)
+    sim.init()
+    sim.step(4000)
+    er = _equilibration_ratios(sim, c, kT, 20000, 200)
+    print("bgk", tau, "ER(rho, j, Pi_aa, Pi_ab) =", np.round(er, 4))
+    assert np.abs(er - 1.0).max() < 0.005, er
 
 
 def test_largest_lattice_768_in_place_sampled_against_oracle():
@@ -298,7 +347,9 @@ def test_fig1_fig2_fluctuation_spectra_256(tau):
         # stability limit, the mid-range shells sit a few per cent ABOVE 1 (the printed means over 24 <= |k| <= 64; rho:
         # 1.03): the direction of the excess Table III prints for tau = 0.51 (1.005 / 1.013 / 1.004 / 1.012 lattice-wide,
         # i.e. averaged up to the Nyquist corner).  Fig.1(c) itself is not in the container, so the 6 % is this build's
-        # bracket, not the paper's.
+        # bracket, not the paper's.  That the excess is the METHOD's and not the kernel's is shown on the oracle:
+        # tests/test_oracle_physics.py::test_tau_051_midshell_density_excess_belongs_to_the_method (1.02 on the same
+        # |k| at 32^3) and test_tau_051_midshell_excess_gpu_equals_oracle_32 below.
         syst = 0.06 if tau < 0.55 else 0.01
         tol = 4.0 / np.sqrt(n_eff * mult * cnt[sel] / 2.0) + syst
         print(name, tau, "ER(|k|=4..64): min %.4f max %.4f" % (er.min(), er.max()), "worst/tol %.2f" % (np.abs(er - 1) / tol).max(),
@@ -306,3 +357,30 @@ def test_fig1_fig2_fluctuation_spectra_256(tau):
         if not (np.abs(er - 1.0) < tol).all() or np.abs(er[20:] - 1.0).max() > syst + 0.01:
             bad.append(name)
     assert not bad, bad
+
+
+def test_tau_051_midshell_excess_gpu_equals_oracle_32():
+    """The few-per-cent density excess on the mid shells at tau = 0.51 (bracketed at 6 % in the 256^3 test above) is
+    the method's: on a 32^3 box the CUDA path and the oracle, started from the same thermal populations with the same
+    seed, give the same shell spectra to 1e-9 (and the same populations to 1e-11 after 1200 steps), and both show the
+    excess on shells 3..8 (tests/test_oracle_physics.py pins the oracle's value over a longer run)."""
+    torch = torch_()
+    n, kT, tau = 32, 1.0 / 3000.0, 0.51
+    w = oracle.tables()[1]
+    f0 = synthetic.gaussian_population_field(n, n, n, 1234, w, np.sqrt(3.0 * kT * w))
+    sim = binding.Rflbm(n, n, n, tau, kT, 1.0, 21)
+    ref = oracle.Ref(n, n, n, tau, kT, 1.0, 21, threads=oracle.max_threads())
+    sim.set_populations(torch.from_numpy(f0), 0); ref.set_populations(f0, 0)
+    sim.step(200); ref.step(200)
+    acc_g, acc_r, ns = 0.0, 0.0, 0
+    while sim.step_count <= 1200:
+        tot_g, cnt = shell_spectrum(sim.moments()[0].cpu().numpy())
+        tot_r, _ = shell_spectrum(ref.moments()[0])
+        acc_g, acc_r, ns = acc_g + tot_g / (3 * kT), acc_r + tot_r / (3 * kT), ns + 1
+        sim.step(50); ref.step(50)
+    assert np.abs(sim.get_populations().cpu().numpy() - ref.get_populations()).max() < 1e-11
+    assert np.abs(acc_g[1:] / acc_r[1:] - 1.0).max() < 1e-9
+    mid_g = acc_g[3:9].sum() / (ns * cnt[3:9].sum())
+    mid_r = acc_r[3:9].sum() / (ns * cnt[3:9].sum())
+    print(f"32^3 tau=0.51 ER_rho shells 3..8: CUDA {mid_g:.5f}, oracle {mid_r:.5f}")
+    assert mid_g > 1.005 and mid_r > 1.005

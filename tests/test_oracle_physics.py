@@ -150,3 +150,31 @@ def test_stable_and_equilibrated_at_extreme_tau(tau):
         r.step(10)
     vs = np.mean(vs, axis=0)
     assert np.abs(vs - 1.0).max() < 0.04, vs
+
+
+def test_tau_051_midshell_density_excess_belongs_to_the_method():
+    """at tau = 0.51 the GPU run at 256^3 keeps the density shells 24 <= |k| <= 64 a few per cent
+    ABOVE their equipartition value (tests/test_gpu_configs.py::test_fig1_fig2_fluctuation_spectra_256 brackets it at
+    6 %).  The ORACLE shows the same excess on the corresponding shells of a 32^3 box (|k| L/2pi = 3..8, the same
+    |k| in lattice units), from the same kind of thermal start: it is a property of the scheme next to the stability
+    limit - the direction Table III prints for tau = 0.51 (1.005 / 1.013 / 1.004 / 1.012 lattice-wide)
+    - and not of the CUDA kernel.  Statistical error of the shell mean: ~0.6 % (1.3e3 independent modes, ~20
+    decorrelated snapshots), so the 1.008 .. 1.05 window is a > 2 sigma statement on both sides; measured 1.020.
+    The whole lattice stays within 1 % of equipartition (measured 1.004), as Table III says."""
+    n, kT, tau = 32, 1.0 / 3000.0, 0.51
+    w = oracle.tables()[1]
+    r = oracle.Ref(n, n, n, tau, kT, 1.0, 21, threads=oracle.max_threads())
+    r.set_populations(synthetic.gaussian_population_field(n, n, n, 1234, w, np.sqrt(3.0 * kT * w)), 0)
+    r.step(200)
+    acc, ns, cnt = 0.0, 0, None
+    while r.step_count <= 2200:
+        rho, _ = r.moments()
+        tot, cnt = shell_spectrum(rho)
+        acc = acc + tot / (3.0 * kT)
+        ns += 1
+        r.step(50)
+    mid = acc[3:9].sum() / (ns * cnt[3:9].sum())
+    whole = acc[1:].sum() / (ns * cnt[1:].sum())
+    print(f"oracle 32^3 tau=0.51: ER_rho shells 3..8 = {mid:.4f}, all shells = {whole:.4f}")
+    assert 1.008 < mid < 1.05, mid
+    assert abs(whole - 1.0) < 0.01, whole
