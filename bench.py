@@ -45,6 +45,7 @@ def parse_args():
     p.add_argument("--impl", default="ours", choices=["ours", "reference"])
     # development knobs (the driver does not pass them)
     p.add_argument("--size", type=int, default=WORKLOAD["size"])
+    p.add_argument("--shape", default=None, help="nx,ny,nz instead of --size^3")
     p.add_argument("--kT", type=float, default=WORKLOAD["kT"])
     p.add_argument("--precision", default="f64", choices=["f64", "f32"])
     p.add_argument("--variant", default="auto", choices=["auto", "plain", "tma"])
@@ -52,6 +53,7 @@ def parse_args():
     p.add_argument("--scheme", default="ab", choices=["ab", "aa"])
     p.add_argument("--no-e2e", action="store_true")
     p.add_argument("--no-sustained", action="store_true")
+    p.add_argument("--e2e-serial", action="store_true")
     p.add_argument("--no-cpu", action="store_true")
     p.add_argument("--cpu-seconds", type=float, default=12.0)
     return p.parse_args()
@@ -228,12 +230,13 @@ def run_ours(args):
     dev = torch.device(f"cuda:{local}")
     torch.cuda.set_device(dev)
     n = args.size
+    nx, ny, nz = (int(v) for v in args.shape.split(",")) if args.shape else (n, n, n)
     prec = binding.F64 if args.precision == "f64" else binding.F32
     es = 8 if prec == binding.F64 else 4
-    N = n ** 3
+    N = nx * ny * nz
     K, W = args.steps, max(3, args.warmup)
 
-    sim = binding.Rflbm(n, n, n, WORKLOAD["tau"], args.kT, WORKLOAD["rho0"], WORKLOAD["seed"], prec, device=dev,
+    sim = binding.Rflbm(nx, ny, nz, WORKLOAD["tau"], args.kT, WORKLOAD["rho0"], WORKLOAD["seed"], prec, device=dev,
                         scheme=binding.SCHEME_AA if args.scheme == "aa" else binding.SCHEME_AB)
     sim.set_kernel_variant({"auto": binding.KERNEL_AUTO, "plain": binding.KERNEL_PLAIN, "tma": binding.KERNEL_TMA}[args.variant])
     if args.model == "bgk":
@@ -286,13 +289,15 @@ def run_ours(args):
     # ---- end to end through the C-ABI with HOST buffers
     e2e = None
     if not args.no_e2e:
-        shape = (n, n, n)
+        shape = (nz, ny, nx)
         dt = torch.float64 if prec == binding.F64 else torch.float32
         rho_h = torch.full(shape, WORKLOAD["rho0"], dtype=dt).pin_memory()
         u_h = torch.zeros((3,) + shape, dtype=dt).pin_memory()
         rho_o = torch.empty(shape, dtype=dt).pin_memory()
         u_o = torch.empty((3,) + shape, dtype=dt).pin_memory()
         scratch = torch.empty(4 * N * es, dtype=torch.uint8, device=dev)
+        copy_stream = torch.cuda.Stream(device=dev)
+        sim.set_copy_stream(None if args.e2e_serial else copy_stream)  # pipelined over z chunks unless --e2e-serial
         sim.run_host(rho_h, u_h, 2, rho_o, u_o, scratch)              # warm the copy path
         barrier_all(); torch.cuda.synchronize(dev)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -303,8 +308,12 @@ def run_ours(args):
         ms_e = max_over_ranks(e0.elapsed_time(e1), dev)
         e2e = {"value": N * K * world / (ms_e * 1e-3) / 1e6, "unit": UNIT,
                "h2d_bytes_per_step": 4 * N * es / K, "d2h_bytes_per_step": 4 * N * es / K,
-               "ms_total": ms_e, "what": "rflbm_run_host: pinned host rho,u -> device, init, K steps, moments, "
-                                         "device -> pinned host, stream sync; bytes are per job / K"}
+               "ms_total": ms_e, "pipelined": not args.e2e_serial,
+               "what": "rflbm_run_host: pinned host rho,u -> device, init, K steps, moments, device -> pinned host, "
+                       "sync; bytes are per job / K; copies on a second stream, z-chunked and overlapped with the "
+                       "kernels (include/rflbm.h)" if not args.e2e_serial else
+                       "rflbm_run_host, serial form: pinned host rho,u -> device, init, K steps, moments, device -> "
+                       "pinned host, sync; bytes are per job / K"}
         assert abs(float(rho_o.double().mean()) / WORKLOAD["rho0"] - 1.0) < 1e-9
         del rho_h, u_h, rho_o, u_o, scratch
 
@@ -315,7 +324,7 @@ def run_ours(args):
     bytes_per_launch = 2 * 27 * es * N
     achieved = bytes_per_launch / (ms_local / K * 1e-3) / 1e9
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": ncu_traffic_bytes(n, args.precision, args.scheme, args.model, kernel) if args.kT > 0 else None,
+                "traffic": ncu_traffic_bytes(n, args.precision, args.scheme, args.model, kernel) if (args.kT > 0 and not args.shape) else None,
                 "peak_source": peak_src, "kernel": kernel,
                 "algorithmic_bytes_per_launch": bytes_per_launch,
                 "avg_launch_ms": ms_local / K}
@@ -334,9 +343,9 @@ def run_ours(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": args.precision, "data": "synthetic",
-        "config": {"workload": f"{n}^3 periodic D3Q27 {'BGK-FLBM' if args.model == 'bgk' else 'Reg-FLBM'} {args.precision}, "
+        "config": {"workload": f"{nx}x{ny}x{nz} periodic D3Q27 {'BGK-FLBM' if args.model == 'bgk' else 'Reg-FLBM'} {args.precision}, "
                                f"rho0=1, u=0, tau=0.8, kT={args.kT:g}, seed 11"
-                               + (" (BASELINE configs[3])" if (n, args.precision, args.model, args.kT) == (512, "f64", "reg", 1e-4) else "")
+                               + (" (BASELINE configs[3])" if (nx, ny, nz, args.precision, args.model, args.kT) == (512, 512, 512, "f64", "reg", 1e-4) else "")
                                + (f"; A-B double buffer {2 * 27 * es * N / 1e9:.1f} GB" if args.scheme == "ab"
                                   else f"; in-place AA buffer {27 * es * N / 1e9:.1f} GB"),
                    "scheme": args.scheme, "model": args.model, "kernel_variant": args.variant,

@@ -165,11 +165,23 @@ int rflbm_set_populations(rflbm_t* h, const void* f_dev, uint64_t step);
 int rflbm_debug_rng(rflbm_t* h, uint64_t step, void* words_dev, void* normals_dev);
 
 /* End-to-end job with HOST buffers (what bench.py's "e2e" times): copy rho_host[N], u_host[3][N] (`real`,
- * ideally pinned) to the device scratch, init, advance nsteps, compute moments, copy them back to
- * rho_out_host / u_out_host and synchronise.  scratch_dev: caller-owned device buffer of at least
- * 4*N*sizeof(real) bytes.  rho_host = u_host = NULL -> uniform rho0, u=0 start (no upload). */
+ * pinned if the copies are to be asynchronous) to the device scratch, init, advance nsteps, compute moments, copy them
+ * back to rho_out_host / u_out_host and synchronise.  scratch_dev: caller-owned device buffer of at least
+ * 4*N*sizeof(real) bytes.  rho_host = u_host = NULL -> uniform rho0, u=0 start (no upload).
+ * Afterwards the handle is in the state rflbm_init + rflbm_step(nsteps) leaves it in.
+ * With a copy stream (rflbm_set_copy_stream) and the A-B scheme the job is PIPELINED over up to 32 chunks of z layers:
+ * a chunk is initialised as soon as it and its two neighbours have been uploaded, a chunk that has done L steps takes
+ * step L+1 as soon as both neighbours have done L (the steps run behind the upload front), and the moments of a chunk
+ * that has finished are downloaded while the others are still stepping.  Every launch is the same kernel restricted to
+ * a z range, so the results are bit-identical to the serial form.  Without a copy stream, in the AA scheme, or with
+ * nz < 3, everything runs one after the other on the handle's stream.  ESTATE in slab mode. */
 int rflbm_run_host(rflbm_t* h, const void* rho_host, const void* u_host, int nsteps, void* rho_out_host,
                    void* u_out_host, void* scratch_dev, size_t scratch_bytes);
+
+/* A second cudaStream_t (as void*), borrowed, on which rflbm_run_host issues its host<->device copies so that they
+ * overlap the kernels on the handle's stream (the two are ordered by events the call creates and destroys).
+ * NULL (the default) or the handle's own stream: rflbm_run_host runs serially.  No other call uses it. */
+int rflbm_set_copy_stream(rflbm_t* h, void* cuda_stream);
 
 /* Number of kernels the handle has launched so far (bench.py's gpu_launches). */
 uint64_t rflbm_launch_count(const rflbm_t* h);

@@ -48,6 +48,7 @@ SYMBOLS = {
     "rflbm_set_populations": (_i32, [_vp, _vp, _u64]),
     "rflbm_debug_rng": (_i32, [_vp, _u64, _vp, _vp]),
     "rflbm_run_host": (_i32, [_vp, _vp, _vp, _i32, _vp, _vp, _vp, _sz]),
+    "rflbm_set_copy_stream": (_i32, [_vp, _vp]),
     "rflbm_launch_count": (_u64, [_vp]),
     "rflbm_last_kernel": (C.c_char_p, [_vp]),
     "rflbm_step_count": (_u64, [_vp]),
@@ -226,8 +227,14 @@ class Rflbm:
             self._ck(self.lib.rflbm_debug_rng(self.h, int(step), words.data_ptr(), normals.data_ptr()))
         return words, normals
 
+    def set_copy_stream(self, stream):
+        """second torch stream for the copies of run_host (None: serial)"""
+        self._copy_stream = stream
+        self._ck(self.lib.rflbm_set_copy_stream(self.h, stream.cuda_stream if stream is not None else None))
+
     def run_host(self, rho_host, u_host, nsteps, rho_out_host, u_out_host, scratch=None):
-        """End-to-end job on HOST tensors (pinned for speed): upload, init, step, moments, download, sync."""
+        """End-to-end job on HOST tensors (pinned for speed): upload, init, step, moments, download, sync;
+        pipelined over z chunks when a copy stream has been set (include/rflbm.h)."""
         t = self.torch
         es = 8 if self.precision == F64 else 4
         with self._ctx():

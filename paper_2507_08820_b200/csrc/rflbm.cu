@@ -29,6 +29,9 @@ static void set_layout(rflbm* h)
     h->QS = (ns + 31) / 32 * 32 + pad;
 }
 
+// launch grid of the one-thread-per-site kernels over the owned layers [zc, zc+zn) of the next launch
+static dim3 zgrid(const rflbm* h) { return dim3(h->grid.x, h->grid.y, (unsigned)h->zn); }
+
 static int fail(rflbm* h, int code, const char* fmt, ...)
 {
     if (h) {
@@ -108,7 +111,15 @@ extern "C" int rflbm_create(int nx, int ny, int nz, double tau, double kT, doubl
     // (16-byte aligned box starts) and every warp's stores are line aligned; tiny lattices stay packed
     const int line = 128 / (int)real_size(h);
     h->px = (nx >= TMA_MIN_NX) ? (nx + line - 1) / line * line : nx;
-    h->tma_tx = nx >= 128 ? 128 : nx >= 64 ? 64 : nx >= TMA_MIN_NX ? 32 : 0;
+    // tile width of the TMA kernel: the one that wastes the fewest threads on the ragged last tile, the widest on a tie
+    h->tma_tx = 0;
+    if (nx >= TMA_MIN_NX) {
+        long long best = -1;
+        for (int tx = 128; tx >= 32; tx /= 2) {
+            const long long covered = (long long)((nx + tx - 1) / tx) * tx;
+            if (best < 0 || covered < best) { best = covered; h->tma_tx = tx; }
+        }
+    }
     set_layout(h);
     if ((double)h->QS >= 4294967296.0) { delete h; return RFLBM_EINVAL; }
     h->nzg = nz;
@@ -116,6 +127,7 @@ extern "C" int rflbm_create(int nx, int ny, int nz, double tau, double kT, doubl
     h->grid = dim3((nx + bx - 1) / bx, (ny + by - 1) / by, nz);
     h->tma_rows = 16;
     h->last_kernel = "";
+    h->zc = 0; h->zn = nz;
     *out = h;
     return RFLBM_OK;
 }
@@ -240,13 +252,13 @@ static int gather_mode(const rflbm* h)
     do {                                                                                                          \
         const int gm_ = gather_mode(h);                                                                           \
         if (h->walls) {                                                                                           \
-            if (gm_ == GATHER_AB) KERNEL<real, true, GATHER_AB><<<h->grid, h->block, 0, h->stream>>>(__VA_ARGS__);       \
-            else if (gm_ == GATHER_AA1) KERNEL<real, true, GATHER_AA1><<<h->grid, h->block, 0, h->stream>>>(__VA_ARGS__); \
-            else KERNEL<real, true, GATHER_AA0><<<h->grid, h->block, 0, h->stream>>>(__VA_ARGS__);                       \
+            if (gm_ == GATHER_AB) KERNEL<real, true, GATHER_AB><<<zgrid(h), h->block, 0, h->stream>>>(__VA_ARGS__);       \
+            else if (gm_ == GATHER_AA1) KERNEL<real, true, GATHER_AA1><<<zgrid(h), h->block, 0, h->stream>>>(__VA_ARGS__); \
+            else KERNEL<real, true, GATHER_AA0><<<zgrid(h), h->block, 0, h->stream>>>(__VA_ARGS__);                       \
         } else {                                                                                                  \
-            if (gm_ == GATHER_AB) KERNEL<real, false, GATHER_AB><<<h->grid, h->block, 0, h->stream>>>(__VA_ARGS__);      \
-            else if (gm_ == GATHER_AA1) KERNEL<real, false, GATHER_AA1><<<h->grid, h->block, 0, h->stream>>>(__VA_ARGS__); \
-            else KERNEL<real, false, GATHER_AA0><<<h->grid, h->block, 0, h->stream>>>(__VA_ARGS__);                      \
+            if (gm_ == GATHER_AB) KERNEL<real, false, GATHER_AB><<<zgrid(h), h->block, 0, h->stream>>>(__VA_ARGS__);      \
+            else if (gm_ == GATHER_AA1) KERNEL<real, false, GATHER_AA1><<<zgrid(h), h->block, 0, h->stream>>>(__VA_ARGS__); \
+            else KERNEL<real, false, GATHER_AA0><<<zgrid(h), h->block, 0, h->stream>>>(__VA_ARGS__);                      \
         }                                                                                                         \
     } while (0)
 
@@ -271,10 +283,10 @@ static int do_init(rflbm* h, const void* rho, const void* u)
 {
     const FieldParams<real> P = field_params<real>(h);
     if (h->walls)
-        init_kernel<real, true><<<h->grid, h->block, 0, h->stream>>>((const real*)rho, (const real*)u, h->rho0,
+        init_kernel<real, true><<<zgrid(h), h->block, 0, h->stream>>>((const real*)rho, (const real*)u, h->rho0,
                                                                       (real*)h->buf[0], (real*)h->buf[1], P);
     else
-        init_kernel<real, false><<<h->grid, h->block, 0, h->stream>>>((const real*)rho, (const real*)u, h->rho0,
+        init_kernel<real, false><<<zgrid(h), h->block, 0, h->stream>>>((const real*)rho, (const real*)u, h->rho0,
                                                                        (real*)h->buf[0], (real*)h->buf[1], P);
     return after_launch(h, "init_kernel");
 }
@@ -299,9 +311,9 @@ static int do_import(rflbm* h, const void* f)
 {
     const FieldParams<real> P = field_params<real>(h);
     if (h->walls)
-        import_kernel<real, true><<<h->grid, h->block, 0, h->stream>>>((const real*)f, (real*)h->buf[0], (real*)h->buf[1], P);
+        import_kernel<real, true><<<zgrid(h), h->block, 0, h->stream>>>((const real*)f, (real*)h->buf[0], (real*)h->buf[1], P);
     else
-        import_kernel<real, false><<<h->grid, h->block, 0, h->stream>>>((const real*)f, (real*)h->buf[0], (real*)h->buf[1], P);
+        import_kernel<real, false><<<zgrid(h), h->block, 0, h->stream>>>((const real*)f, (real*)h->buf[0], (real*)h->buf[1], P);
     return after_launch(h, "import_kernel");
 }
 
@@ -376,8 +388,10 @@ static void dispatch_step(rflbm* h, const StepParams<real>& P, int variant, int 
     else dispatch_tile<real, STEP_AA_ODD>(h, P, variant, tx);
 }
 
+// one launch of the step kernel at time h->t over the owned layers [h->zc, h->zc + h->zn), reading buf[h->cur];
+// no state change
 template <typename real>
-static int do_step(rflbm* h, int nsteps)
+static int launch_step_once(rflbm* h)
 {
     const bool noise = h->kT > 0.0;       // kT = 0: deterministic (Reg-)LBM, RNG skipped entirely (R17)
     if (h->variant == RFLBM_KERNEL_TMA && !h->tma_ok)
@@ -386,11 +400,17 @@ static int do_step(rflbm* h, int nsteps)
     const bool ghost = h->model == RFLBM_MODEL_REG && h->tau_g != 1.0;
     const int variant = (ghost ? 16 : 0) | (h->model == RFLBM_MODEL_BGK ? 8 : 0) | (h->walls ? 4 : 0) | (h->force ? 2 : 0) | (noise ? 1 : 0);
     static const char* const names[4] = {"step_kernel", "step_kernel_tma<TX=32>", "step_kernel_tma<TX=64>", "step_kernel_tma<TX=128>"};
+    const StepParams<real> P = step_params<real>(h, h->t);
+    dispatch_step<real>(h, P, variant, tma ? h->tma_tx : 0);
+    h->last_kernel = !tma ? names[0] : h->tma_tx == 32 ? names[1] : h->tma_tx == 64 ? names[2] : names[3];
+    return after_launch(h, h->last_kernel);
+}
+
+template <typename real>
+static int do_step(rflbm* h, int nsteps)
+{
     for (int s = 0; s < nsteps; ++s) {
-        const StepParams<real> P = step_params<real>(h, h->t);
-        dispatch_step<real>(h, P, variant, tma ? h->tma_tx : 0);
-        h->last_kernel = !tma ? names[0] : h->tma_tx == 32 ? names[1] : h->tma_tx == 64 ? names[2] : names[3];
-        const int rc = after_launch(h, h->last_kernel);
+        const int rc = launch_step_once<real>(h);
         if (rc != RFLBM_OK) return rc;
         if (h->scheme == RFLBM_SCHEME_AB) h->cur ^= 1;
         else h->aa_phase ^= 1;
@@ -495,11 +515,11 @@ extern "C" int rflbm_debug_rng(rflbm_t* h, uint64_t step, void* words_dev, void*
     const uint32_t t_hi = (uint32_t)(step >> 32), t_lo = (uint32_t)(step & 0xFFFFFFFFu);
     if (h->precision == RFLBM_F64) {
         const StepParams<double> P = step_params<double>(h, step);
-        debug_rng_kernel<double><<<h->grid, h->block, 0, h->stream>>>((uint32_t*)words_dev, (double*)normals_dev,
+        debug_rng_kernel<double><<<zgrid(h), h->block, 0, h->stream>>>((uint32_t*)words_dev, (double*)normals_dev,
                                                                      mismatch, t_hi, t_lo, P);
     } else {
         const StepParams<float> P = step_params<float>(h, step);
-        debug_rng_kernel<float><<<h->grid, h->block, 0, h->stream>>>((uint32_t*)words_dev, (float*)normals_dev,
+        debug_rng_kernel<float><<<zgrid(h), h->block, 0, h->stream>>>((uint32_t*)words_dev, (float*)normals_dev,
                                                                     mismatch, t_hi, t_lo, P);
     }
     rc = after_launch(h, "debug_rng_kernel");
@@ -514,18 +534,10 @@ extern "C" int rflbm_debug_rng(rflbm_t* h, uint64_t step, void* words_dev, void*
 }
 
 // ---------------------------------------------------------------- host-buffer job (bench.py "e2e")
-extern "C" int rflbm_run_host(rflbm_t* h, const void* rho_host, const void* u_host, int nsteps, void* rho_out_host,
-                              void* u_out_host, void* scratch_dev, size_t scratch_bytes)
+// Serial form: everything on the handle's stream, one copy after the other.
+static int run_host_serial(rflbm* h, const void* rho_host, const void* u_host, int nsteps, void* rho_out_host,
+                           void* u_out_host, char* d_rho, char* d_u, size_t fb)
 {
-    if (!h) return RFLBM_EINVAL;
-    if (!rho_out_host || !u_out_host || !scratch_dev) return fail(h, RFLBM_EINVAL, "NULL output or scratch pointer");
-    if ((rho_host == nullptr) != (u_host == nullptr))
-        return fail(h, RFLBM_EINVAL, "rho_host and u_host must both be given or both NULL");
-    if (h->slab) return fail(h, RFLBM_ESTATE, "rflbm_run_host is a whole-lattice job: not available in slab mode");
-    const size_t fb = (size_t)h->N * real_size(h);
-    if (scratch_bytes < 4 * fb) return fail(h, RFLBM_ENOMEM, "scratch too small: %zu < %zu bytes", scratch_bytes, 4 * fb);
-    char* d_rho = (char*)scratch_dev;
-    char* d_u = d_rho + fb;
     int rc;
     if (rho_host) {
         rc = check_cuda(h, cudaMemcpyAsync(d_rho, rho_host, fb, cudaMemcpyHostToDevice, h->stream), "H2D rho");
@@ -546,6 +558,183 @@ extern "C" int rflbm_run_host(rflbm_t* h, const void* rho_host, const void* u_ho
     rc = check_cuda(h, cudaMemcpyAsync(u_out_host, d_u, 3 * fb, cudaMemcpyDeviceToHost, h->stream), "D2H u");
     if (rc != RFLBM_OK) return rc;
     return check_cuda(h, cudaStreamSynchronize(h->stream), "cudaStreamSynchronize");
+}
+
+// Pipelined form (A-B scheme, a copy stream given): the lattice is cut into C chunks of consecutive z layers.  The
+// copies run on the copy stream, the kernels on the handle's stream, ordered by events:
+//   * chunk c of (rho, u) is uploaded, and as soon as chunks c-1, c, c+1 are on the device chunk c is initialised;
+//   * a chunk that has done L steps may do step L+1 once both neighbours have done at least L (the pull reads one
+//     layer of each neighbour; the A-B buffer that step L+1 overwrites held level L-1, which nobody needs any more):
+//     the steps start behind the upload front and form a pyramid in (z, t) while the rest is still on the wire;
+//   * at the end the chunks are brought to step K one after the other (each needs a cone of its neighbours), and the
+//     moments of a finished chunk are computed and downloaded while the others are still stepping.
+// Every launch is the same kernel restricted to a z range (Geom::zc), so the result is bit-identical to the serial form.
+namespace {
+struct Pipeline {
+    rflbm* h;
+    int C, CH, K;
+    int* level;                   // -1: not initialised, L >= 0: L steps done
+    cudaEvent_t* up;              // chunk uploaded
+    const void *d_rho, *d_u;      // device fields for init (NULL: uniform start)
+    int rc;
+    int za(int c) const { return c * CH; }
+    int zn(int c) const { return (c == C - 1) ? h->nz - c * CH : CH; }
+    int prev(int c) const { return (c + C - 1) % C; }
+    int next(int c) const { return (c + 1) % C; }
+    void range(int c) { h->zc = za(c); h->zn = zn(c); }
+    template <typename real> void init(int c)
+    {
+        if (rc != RFLBM_OK) return;
+        range(c);
+        rc = do_init<real>(h, d_rho, d_u);
+        level[c] = 0;
+    }
+    template <typename real> void step(int c)
+    {
+        if (rc != RFLBM_OK) return;
+        range(c);
+        h->t = (uint64_t)level[c];
+        h->cur = level[c] & 1;
+        rc = launch_step_once<real>(h);
+        level[c] += 1;
+    }
+    bool can_step(int c) const
+    {
+        return level[c] >= 0 && level[c] < K && level[prev(c)] >= level[c] && level[next(c)] >= level[c];
+    }
+    // everything that is possible right now, lowest levels first (the pyramid behind the upload front)
+    template <typename real> void greedy()
+    {
+        for (bool progressed = true; progressed && rc == RFLBM_OK;) {
+            progressed = false;
+            for (int c = 0; c < C; ++c)
+                if (can_step(c)) { step<real>(c); progressed = true; }
+        }
+    }
+    // bring chunk c to level L (all chunks are initialised): its neighbours first, one level below
+    template <typename real> void advance_to(int c, int L)
+    {
+        while (level[c] < L && rc == RFLBM_OK) {
+            advance_to<real>(prev(c), level[c]);
+            advance_to<real>(next(c), level[c]);
+            step<real>(c);
+        }
+    }
+};
+}  // namespace
+
+template <typename real>
+static int run_host_pipelined(rflbm* h, const void* rho_host, const void* u_host, int nsteps, void* rho_out_host,
+                              void* u_out_host, char* d_rho, char* d_u, size_t fb)
+{
+    const size_t es = sizeof(real);
+    // 32 chunks: measured at 512^3, K = 20 (e2e ms): 16 chunks 308, 24: 284, 32: 271, 64: 293 — finer chunks make
+    // a taller pyramid of steps behind the upload front, but smaller launches fill the 148 SMs worse
+    constexpr int MAXC = 32;
+    const int CH = (h->nz + MAXC - 1) / MAXC, C = (h->nz + CH - 1) / CH;
+    const size_t layer = (size_t)h->nx * h->ny * es;
+    int level[MAXC];
+    cudaEvent_t up[MAXC], mom[MAXC];
+    for (int c = 0; c < C; ++c) {
+        level[c] = -1;
+        cudaEventCreateWithFlags(&up[c], cudaEventDisableTiming);
+        cudaEventCreateWithFlags(&mom[c], cudaEventDisableTiming);
+    }
+    Pipeline p{h, C, CH, nsteps, level, up, rho_host ? d_rho : nullptr, rho_host ? d_u : nullptr, RFLBM_OK};
+    // a chunk launch is 1/32 of the lattice: finer blocks (8 rows instead of 16) keep its last wave of blocks short
+    const int rows_full = h->tma_rows;
+    h->tma_rows = 8;
+    cudaStream_t cs = h->copy_stream;
+    int rc = RFLBM_OK;
+    // the copy stream starts after whatever the caller has already enqueued on the handle's stream
+    cudaEvent_t start;
+    cudaEventCreateWithFlags(&start, cudaEventDisableTiming);
+    cudaEventRecord(start, h->stream);
+    cudaStreamWaitEvent(cs, start, 0);
+    // ---- uploads, in z order
+    for (int c = 0; c < C && rc == RFLBM_OK; ++c) {
+        if (rho_host) {
+            const size_t off = (size_t)p.za(c) * layer, len = (size_t)p.zn(c) * layer;
+            rc = check_cuda(h, cudaMemcpyAsync(d_rho + off, (const char*)rho_host + off, len, cudaMemcpyHostToDevice, cs), "H2D rho");
+            for (int k = 0; k < 3 && rc == RFLBM_OK; ++k)
+                rc = check_cuda(h, cudaMemcpyAsync(d_u + k * fb + off, (const char*)u_host + k * fb + off, len, cudaMemcpyHostToDevice, cs), "H2D u");
+        }
+        cudaEventRecord(up[c], cs);
+    }
+    // ---- init behind the upload front, steps behind the init front
+    for (int a = 2; a < C && rc == RFLBM_OK; ++a) {
+        cudaStreamWaitEvent(h->stream, up[a], 0);          // chunks a-2, a-1, a are on the device
+        p.template init<real>(a - 1);
+        p.template greedy<real>();
+    }
+    p.template init<real>(C - 1);                           // needs chunk 0: the periodic wrap closes the ring last
+    p.template init<real>(0);
+    // ---- finish chunk after chunk; moments and download of a finished chunk overlap the stepping of the others
+    int next_out = 0;
+    auto flush_outputs = [&](int upto) {                   // chunks < upto whose neighbours are finished too
+        for (; next_out < upto && p.rc == RFLBM_OK; ++next_out) {
+            const int c = next_out;
+            p.range(c);
+            h->t = (uint64_t)nsteps; h->cur = nsteps & 1;
+            p.rc = do_moments<real>(h, d_rho, d_u);
+            cudaEventRecord(mom[c], h->stream);
+            cudaStreamWaitEvent(cs, mom[c], 0);
+            const size_t off = (size_t)p.za(c) * layer, len = (size_t)p.zn(c) * layer;
+            cudaMemcpyAsync((char*)rho_out_host + off, d_rho + off, len, cudaMemcpyDeviceToHost, cs);
+            for (int k = 0; k < 3; ++k)
+                cudaMemcpyAsync((char*)u_out_host + k * fb + off, d_u + k * fb + off, len, cudaMemcpyDeviceToHost, cs);
+        }
+    };
+    for (int c = 0; c < C && p.rc == RFLBM_OK; ++c) {
+        p.template advance_to<real>(c, nsteps);
+        if (c >= 1 && c + 1 < C) {                          // chunk c-1 can go out once c-2, c-1, c are finished
+            if (c == 1) p.template advance_to<real>(C - 1, nsteps);   // chunk 0 also needs its other neighbour
+            flush_outputs(c);
+        }
+    }
+    flush_outputs(C);
+    rc = (rc != RFLBM_OK) ? rc : p.rc;
+    // ---- state of the handle: as after rflbm_init + rflbm_step(nsteps)
+    h->zc = 0; h->zn = h->nz;
+    h->tma_rows = rows_full;
+    h->t = (uint64_t)nsteps; h->cur = nsteps & 1; h->aa_phase = 0; h->inited = true;
+    after_state_change(h);
+    cudaError_t e1 = cudaStreamSynchronize(cs), e2 = cudaStreamSynchronize(h->stream);
+    for (int c = 0; c < C; ++c) { cudaEventDestroy(up[c]); cudaEventDestroy(mom[c]); }
+    cudaEventDestroy(start);
+    if (rc != RFLBM_OK) return rc;
+    rc = check_cuda(h, e1, "cudaStreamSynchronize (copy stream)");
+    return rc != RFLBM_OK ? rc : check_cuda(h, e2, "cudaStreamSynchronize");
+}
+
+extern "C" int rflbm_run_host(rflbm_t* h, const void* rho_host, const void* u_host, int nsteps, void* rho_out_host,
+                              void* u_out_host, void* scratch_dev, size_t scratch_bytes)
+{
+    if (!h) return RFLBM_EINVAL;
+    if (!rho_out_host || !u_out_host || !scratch_dev) return fail(h, RFLBM_EINVAL, "NULL output or scratch pointer");
+    if ((rho_host == nullptr) != (u_host == nullptr))
+        return fail(h, RFLBM_EINVAL, "rho_host and u_host must both be given or both NULL");
+    if (nsteps < 0) return fail(h, RFLBM_EINVAL, "nsteps < 0");
+    if (!h->ws) return fail(h, RFLBM_ESTATE, "rflbm_run_host before rflbm_set_workspace");
+    if (h->slab) return fail(h, RFLBM_ESTATE, "rflbm_run_host is a whole-lattice job: not available in slab mode");
+    const size_t fb = (size_t)h->N * real_size(h);
+    if (scratch_bytes < 4 * fb) return fail(h, RFLBM_ENOMEM, "scratch too small: %zu < %zu bytes", scratch_bytes, 4 * fb);
+    char* d_rho = (char*)scratch_dev;
+    char* d_u = d_rho + fb;
+    // the pipeline needs a second stream, the A-B scheme (an odd AA step writes into its neighbours' layers) and at
+    // least three chunks (a chunk's two neighbours must be two different chunks)
+    if (h->copy_stream != nullptr && h->copy_stream != h->stream && h->scheme == RFLBM_SCHEME_AB && h->nz >= 3)
+        return (h->precision == RFLBM_F64)
+                   ? run_host_pipelined<double>(h, rho_host, u_host, nsteps, rho_out_host, u_out_host, d_rho, d_u, fb)
+                   : run_host_pipelined<float>(h, rho_host, u_host, nsteps, rho_out_host, u_out_host, d_rho, d_u, fb);
+    return run_host_serial(h, rho_host, u_host, nsteps, rho_out_host, u_out_host, d_rho, d_u, fb);
+}
+
+extern "C" int rflbm_set_copy_stream(rflbm_t* h, void* cuda_stream)
+{
+    if (!h) return RFLBM_EINVAL;
+    h->copy_stream = (cudaStream_t)cuda_stream;
+    return RFLBM_OK;
 }
 
 extern "C" int rflbm_set_scheme(rflbm_t* h, int scheme)

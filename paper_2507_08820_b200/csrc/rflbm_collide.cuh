@@ -43,6 +43,7 @@ struct Geom {
     int nz;                 // owned layers
     int nzs;                // layers in storage: nz, or nz + 2 in slab mode
     int z_lo;               // storage index of the first owned layer: 0, or 1 in slab mode
+    int zc;                 // first owned layer this LAUNCH works on (0 unless rflbm_run_host pipelines z-chunks), grid.z counts from it
     int zg0;                // global z of storage layer 0: 0, or z0 - 1 in slab mode
     int nzg;                // global number of layers (= nz without a slab)
     int px;                 // row pitch of the internal buffers, in elements

@@ -46,6 +46,8 @@ struct rflbm {
     int variant;          // RFLBM_KERNEL_AUTO / _PLAIN / _TMA
     int tma_rows;         // y rows walked by one block of the TMA kernel
     const char* last_kernel;   // what the last rflbm_step launched (static string)
+    int zc, zn;           // owned layers [zc, zc+zn) the next launch covers (0, nz except inside rflbm_run_host's pipeline)
+    cudaStream_t copy_stream;  // optional second stream for the copies of rflbm_run_host (rflbm_set_copy_stream)
     char err[512];
 };
 
@@ -55,6 +57,7 @@ inline Geom make_geom(const rflbm* h)
     G.nx = h->nx; G.ny = h->ny; G.nz = h->nz;
     G.nzs = h->nz + (h->slab ? 2 : 0);
     G.z_lo = h->slab ? 1 : 0;
+    G.zc = h->zc;
     G.zg0 = h->slab ? h->z0 - 1 : 0;
     G.nzg = h->slab ? h->nzg : h->nz;
     G.px = h->px;
@@ -72,11 +75,12 @@ static inline void launch_one(rflbm* h, const StepParams<real>& P)
     const real* src = (const real*)h->buf[h->cur];
     real* dst = (real*)h->buf[PHASE == STEP_AB ? (h->cur ^ 1) : h->cur];
     if constexpr (TX != 0) {
-        const dim3 grid((h->nx + TX - 1) / TX, (h->ny + h->tma_rows - 1) / h->tma_rows, h->nz);
+        const dim3 grid((h->nx + TX - 1) / TX, (h->ny + h->tma_rows - 1) / h->tma_rows, h->zn);
         step_kernel_tma<real, TX, WALLS, FORCE, NOISE, BGK, GHOST, PHASE><<<grid, BLOCK_T, 0, h->stream>>>(
             h->tmap[h->cur], src, dst, P, h->tma_rows);
     } else {
-        step_kernel<real, WALLS, FORCE, NOISE, BGK, GHOST, PHASE><<<h->grid, h->block, 0, h->stream>>>(src, dst, P);
+        const dim3 grid(h->grid.x, h->grid.y, h->zn);
+        step_kernel<real, WALLS, FORCE, NOISE, BGK, GHOST, PHASE><<<grid, h->block, 0, h->stream>>>(src, dst, P);
     }
 }
 

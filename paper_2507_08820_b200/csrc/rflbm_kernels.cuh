@@ -31,11 +31,12 @@ __device__ __forceinline__ SiteIndex my_site(const Geom& G)
     SiteIndex i;
     i.x = blockIdx.x * blockDim.x + threadIdx.x;
     i.y = blockIdx.y * blockDim.y + threadIdx.y;
-    i.z = (int)blockIdx.z + G.z_lo;
+    const int zl = (int)blockIdx.z + G.zc;                  // owned-layer index
+    i.z = zl + G.z_lo;
     i.zg = i.z + G.zg0;
     i.valid = (i.x < G.nx) && (i.y < G.ny);
     i.s = (long long)i.x + (long long)G.px * i.y + G.pxy * i.z;
-    i.sl = (long long)i.x + (long long)G.nx * ((long long)i.y + (long long)G.ny * (long long)blockIdx.z);
+    i.sl = (long long)i.x + (long long)G.nx * ((long long)i.y + (long long)G.ny * (long long)zl);
     i.site = (uint32_t)((long long)i.x + (long long)G.nx * ((long long)i.y + (long long)G.ny * (long long)i.zg));
     return i;
 }
@@ -282,7 +283,7 @@ import_kernel(const real* __restrict__ in, real* __restrict__ bufA, real* __rest
     if (!i.valid) return;
     const Geom& G = P.G;
     const bool solid = WALLS && solid_layer(G, i.zg);
-    const int zl = (int)blockIdx.z;
+    const int zl = (int)blockIdx.z + G.zc;
     const long long Nin = (long long)G.nx * G.ny * (G.nz + 2 * P.ghost_in);
 #pragma unroll
     for (int n = 0; n < Q; ++n) {
@@ -325,7 +326,7 @@ init_kernel(const real* __restrict__ rho, const real* __restrict__ u, double rho
     if (!i.valid) return;
     const Geom& G = P.G;
     const bool solid = WALLS && solid_layer(G, i.zg);
-    const int zl = (int)blockIdx.z;
+    const int zl = (int)blockIdx.z + G.zc;
     const long long Nin = (long long)G.nx * G.ny * (G.nz + 2 * P.ghost_in);
 #pragma unroll 1
     for (int q = 0; q < Q; ++q) {

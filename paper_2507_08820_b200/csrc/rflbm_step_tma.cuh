@@ -150,7 +150,7 @@ step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const real* src, r
 #endif
 
     const Geom& G = P.G;
-    const int z = (int)blockIdx.z + G.z_lo, zg = z + G.zg0;
+    const int z = (int)blockIdx.z + G.zc + G.z_lo, zg = z + G.zg0;
     if (WALLS && solid_layer(G, zg)) return;                   // solid layers are never updated
     const int tid = threadIdx.x;
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);    // warp-uniform for the compiler too
@@ -183,11 +183,14 @@ step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const real* src, r
     const real* tile = &s_stage[0] + r * T::ROW_STAGE + xl;
     const bool bounce_lo = WALLS && zg == 1, bounce_hi = WALLS && zg == G.nzg - 2;
     uint32_t parity = 0;
+    // row-invariant parts of the storage index and of the Philox site key (the key is < 2^32: 32-bit arithmetic is exact)
+    const long long s_col = (long long)x + G.pxy * z;
+    const uint32_t site_col = (uint32_t)x + (uint32_t)G.nx * (uint32_t)G.ny * (uint32_t)zg;
 
     for (int yb = y_begin; yb < y_end; yb += T::RB) {
         const int y = yb + r;
         const bool row_ok = (T::RB == 1) || y < y_end;          // warp-uniform
-        const long long s = (long long)x + (long long)G.px * y + G.pxy * z;
+        const long long s = s_col + (long long)G.px * y;
         // periodic wrap in x: TMA zero-fills these 9 values; fetch them early, use them after the barrier
         real wv[3][3];
         if (PHASE != STEP_AA_EVEN && edge_warp && row_ok) {     // warp-uniform branch: interior warps skip all of this
@@ -268,7 +271,7 @@ step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const real* src, r
             }
         }
         if (active && row_ok) {
-            const uint32_t site = (uint32_t)((long long)x + (long long)G.nx * ((long long)y + (long long)G.ny * (long long)zg));
+            const uint32_t site = site_col + (uint32_t)G.nx * (uint32_t)y;
             collide<real, FORCE, NOISE, BGK, GHOST>(g, P, site, s_tab, s_tab + LOG_TABLE_N);
             if (PHASE == STEP_AA_ODD) {
                 // push to the neighbours x + c_q (slot q), misaligned by one element for cx = +-1: the partial

@@ -199,6 +199,48 @@ def test_run_host_matches_device_path():
     assert sim.launch_count == 22                                             # init + 20 steps + moments
 
 
+@pytest.mark.parametrize("shape,prec,walls,force,nsteps", [
+    ((24, 10, 6), binding.F64, False, None, 20), ((40, 6, 70), binding.F64, True, (1e-5, 0.0, 2e-6), 9),
+    ((130, 5, 33), binding.F32, False, None, 13), ((9, 4, 3), binding.F64, False, None, 5),
+    ((36, 4, 40), binding.F64, False, None, 0), ((36, 4, 40), binding.F64, True, None, 1)])
+def test_run_host_pipelined_is_bit_identical_to_serial(shape, prec, walls, force, nsteps):
+    """rflbm_run_host with a copy stream (z-chunked upload / init / steps behind the upload front / chunked download)
+    against the serial form of the same call: bit-identical moments AND bit-identical final state of the handle;
+    chunk sizes 1..3 layers with a ragged last chunk, walls, force, fp32, 0 and 1 steps."""
+    torch = torch_()
+    nx, ny, nz = shape
+    dt = torch.float64 if prec == binding.F64 else torch.float32
+    rho, u = synthetic.smooth_random_fields(nx, ny, nz, 12)
+    rho_h = torch.from_numpy(rho).to(dt).pin_memory(); u_h = torch.from_numpy(u).to(dt).pin_memory()
+    outs = []
+    for piped in (False, True):
+        sim = binding.Rflbm(nx, ny, nz, 0.8, 1e-4, 1.0, 21, prec)
+        if walls:
+            sim.set_walls_z(True)
+        if force is not None:
+            sim.set_force(*force)
+        if piped:
+            sim.set_copy_stream(torch.cuda.Stream())
+        ro = torch.empty_like(rho_h).pin_memory(); uo = torch.empty_like(u_h).pin_memory()
+        sim.run_host(rho_h, u_h, nsteps, ro, uo)
+        assert sim.step_count == nsteps
+        sim.step(3)                                           # the handle continues from the state the job left
+        outs.append((ro.clone(), uo.clone(), sim.get_populations().clone(), sim.launch_count))
+    assert torch.equal(outs[0][0], outs[1][0]) and torch.equal(outs[0][1], outs[1][1])
+    assert torch.equal(outs[0][2], outs[1][2])
+    if nz >= 3:
+        assert outs[1][3] > outs[0][3]                        # the pipelined job really ran chunk by chunk
+    # uniform start without upload
+    a = binding.Rflbm(nx, ny, nz, 0.8, 1e-4, 1.0, 21, prec); b = binding.Rflbm(nx, ny, nz, 0.8, 1e-4, 1.0, 21, prec)
+    b.set_copy_stream(torch.cuda.Stream())
+    res = []
+    for sim in (a, b):
+        ro = torch.empty_like(rho_h).pin_memory(); uo = torch.empty_like(u_h).pin_memory()
+        sim.run_host(None, None, nsteps, ro, uo)
+        res.append((ro, uo))
+    assert torch.equal(res[0][0], res[1][0]) and torch.equal(res[0][1], res[1][1])
+
+
 @pytest.mark.parametrize("shape,walls,force,kT", [((128, 4, 3), False, None, 1e-4), ((256, 5, 4), True, (1e-5, 2e-6, -3e-6), 1e-4),
                                                  ((300, 3, 3), False, None, 1e-4), ((130, 18, 5), True, None, 0.0),
                                                  ((384, 20, 2), False, (1e-6, 0.0, 0.0), 1e-3),
@@ -256,9 +298,10 @@ def test_tma_variant_rejected_only_below_32_and_auto_never_takes_the_plain_kerne
         assert e.value.code == binding.EINVAL
     # AUTO with noise: every lattice with nx >= 32 runs the TMA kernel (the internal row pitch is padded, so odd nx
     # qualifies); kT = 0 keeps the plain kernel (pure streaming, where it is the faster one)
-    for nx, prec, name in ((32, binding.F64, "TX=32"), (33, binding.F32, "TX=32"), (64, binding.F64, "TX=64"),
-                           (127, binding.F32, "TX=64"), (129, binding.F64, "TX=128"), (130, binding.F32, "TX=128"),
-                           (511, binding.F64, "TX=128")):
+    # tile width: fewest idle threads on the ragged last tile, widest on a tie
+    for nx, prec, name in ((32, binding.F64, "TX=32"), (33, binding.F32, "TX=64"), (64, binding.F64, "TX=64"),
+                           (96, binding.F64, "TX=32"), (127, binding.F32, "TX=128"), (129, binding.F64, "TX=32"),
+                           (130, binding.F32, "TX=32"), (200, binding.F64, "TX=32"), (320, binding.F64, "TX=64"), (511, binding.F64, "TX=128")):
         sim = binding.Rflbm(nx, 3, 3, 0.8, 1e-4, precision=prec)
         assert sim.last_kernel == ""
         sim.init(); sim.step(2)

@@ -145,7 +145,7 @@ def test_slab_resume_from_exported_state_and_set_populations():
             s.step(1)
         exchange(slabs)
     assert torch.equal(torch.cat([s.get_populations() for s in slabs], dim=1), one.get_populations())
-    assert slabs[0].last_kernel.startswith("step_kernel_tma<TX=32>") and one.last_kernel == slabs[0].last_kernel
+    assert slabs[0].last_kernel.startswith("step_kernel_tma<TX=64>") and one.last_kernel == slabs[0].last_kernel
     with pytest.raises(binding.RflbmError) as e:
         slabs[0].step(2)                                      # one step at a time in slab mode
     assert e.value.code == binding.EINVAL
