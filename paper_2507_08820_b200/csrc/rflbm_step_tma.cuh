@@ -287,11 +287,11 @@ step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const real* src, r
                     for (int b = 0; b < 3; ++b)
 #pragma unroll
                         for (int a = 0; a < 3; ++a) {
-                            // one IMAD.WIDE.U32 per store: out + QS * sizeof(real) * slot (QS < 2^32: exact 32x32->64)
+                            // out + QS * sizeof(real) * slot as a 32x32->64 product (QS < 2^32): one IMAD.WIDE.U32 with the addend folded in.
+                            // (An inline `mad.wide.u32` came out of ptxas as IMAD.WIDE + IADD3 + IMAD.X: 3 instructions.)
                             const int q = a + 3 * b + 9 * c;
                             const unsigned slot = (PHASE == STEP_AA_EVEN) ? 26 - q : q;
-                            unsigned long long at;
-                            asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(at) : "r"(QS32), "r"((unsigned)sizeof(real) * slot), "l"(out));
+                            const unsigned long long at = out + (unsigned long long)QS32 * ((unsigned)sizeof(real) * slot);
                             __stcs(reinterpret_cast<real*>(at), g[c][b][a]);
                         }
             }
