@@ -247,7 +247,9 @@ def test_run_host_pipelined_is_bit_identical_to_serial(shape, prec, walls, force
                                                  ((129, 7, 5), False, None, 1e-4), ((131, 19, 4), True, (1e-5, 0.0, 0.0), 1e-4),
                                                  ((32, 9, 4), False, None, 1e-4), ((33, 35, 3), True, None, 1e-4),
                                                  ((64, 17, 3), False, (1e-6, 1e-6, 0.0), 1e-4), ((100, 6, 5), True, None, 1e-4),
-                                                 ((127, 33, 2), False, None, 1e-4)])
+                                                 ((127, 33, 2), False, None, 1e-4),
+                                                 ((128, 1, 1), False, None, 1e-4), ((64, 2, 1), False, None, 1e-4),
+                                                 ((33, 1, 2), False, (1e-6, 0.0, 1e-6), 1e-4), ((32, 1, 3), True, None, 1e-4)])
 def test_tma_kernel_matches_plain_kernel_and_oracle(shape, walls, force, kT):
     """The TMA-staged step kernel (fp64; tiles of 128, 64 or 32 sites; any nx >= 32, odd ones included: the internal
     row pitch is padded) against the plain kernel (bit for bit: same arithmetic) and the oracle; shapes span several

@@ -55,6 +55,8 @@ CASES = [
     (136, 4, 7, (3, 4), binding.F32, binding.SCHEME_AA, False, None, 1e-4),
     (9, 7, 5, (5,), binding.F64, binding.SCHEME_AB, False, None, 1e-4),             # one slab: its own neighbour
     (9, 7, 5, (5,), binding.F64, binding.SCHEME_AA, False, None, 0.0),
+    (34, 3, 4, (1, 1, 1, 1), binding.F64, binding.SCHEME_AA, False, None, 1e-4),     # every slab a single layer
+    (34, 3, 4, (1, 1, 1, 1), binding.F64, binding.SCHEME_AB, True, None, 1e-4),
 ]
 
 
