@@ -86,6 +86,64 @@ struct Moments10 {
     real rho, jx, jy, jz, pxx, pyy, pzz, pxy, pxz, pyz;
 };
 
+// Packed fp32 arithmetic (sm_100: FADD2 / FMUL2 / FFMA2 work on two floats in an aligned register pair).  The fp32
+// kernel is issue bound, so the two places where the same operation runs on many independent values - the separable
+// transforms - are written on pairs: the same operations in the same order as the scalar code (bit-identical results).
+__device__ __forceinline__ unsigned long long f2_bits(float2 a) { return *reinterpret_cast<unsigned long long*>(&a); }
+__device__ __forceinline__ float2 f2_from(unsigned long long a) { return *reinterpret_cast<float2*>(&a); }
+__device__ __forceinline__ float2 add2(float2 a, float2 b)
+{
+    unsigned long long d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(f2_bits(a)), "l"(f2_bits(b)));
+    return f2_from(d);
+}
+__device__ __forceinline__ float2 sub2(float2 a, float2 b)
+{
+    unsigned long long d;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(f2_bits(a)), "l"(f2_bits(b)));
+    return f2_from(d);
+}
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c)
+{
+    unsigned long long d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(f2_bits(a)), "l"(f2_bits(b)), "l"(f2_bits(c)));
+    return f2_from(d);
+}
+
+// fp32: the x and y passes run on the pair (cz = -1, cz = +1), the cz = 0 plane on scalars; same sums as below
+__device__ __forceinline__ Moments10<float> forward_moments(const float (&g)[3][3][3])
+{
+    float2 P0[3], P1[3], P2[3];     // [cy]: pair over c = 0, 2
+    float S0[3], S1[3], S2[3];      // c = 1
+#pragma unroll
+    for (int b = 0; b < 3; ++b) {
+        const float2 g0 = make_float2(g[0][b][0], g[2][b][0]), g1 = make_float2(g[0][b][1], g[2][b][1]),
+                     g2 = make_float2(g[0][b][2], g[2][b][2]);
+        P2[b] = add2(g2, g0);
+        P1[b] = sub2(g2, g0);
+        P0[b] = add2(P2[b], g1);
+        S2[b] = g[1][b][2] + g[1][b][0];
+        S1[b] = g[1][b][2] - g[1][b][0];
+        S0[b] = S2[b] + g[1][b][1];
+    }
+    const float2 Y02 = add2(P0[2], P0[0]), Y01 = sub2(P0[2], P0[0]), Y00 = add2(Y02, P0[1]);
+    const float2 Y10 = add2(add2(P1[2], P1[0]), P1[1]), Y11 = sub2(P1[2], P1[0]), Y20 = add2(add2(P2[2], P2[0]), P2[1]);
+    const float y02 = S0[2] + S0[0], y01 = S0[2] - S0[0], y00 = y02 + S0[1];
+    const float y10 = (S1[2] + S1[0]) + S1[1], y11 = S1[2] - S1[0], y20 = (S2[2] + S2[0]) + S2[1];
+    Moments10<float> m;      // .x = plane c = 0, .y = plane c = 2
+    m.pzz = Y00.y + Y00.x;
+    m.jz = Y00.y - Y00.x;
+    m.rho = m.pzz + y00;
+    m.jy = (Y01.y + Y01.x) + y01;
+    m.pyz = Y01.y - Y01.x;
+    m.pyy = (Y02.y + Y02.x) + y02;
+    m.jx = (Y10.y + Y10.x) + y10;
+    m.pxz = Y10.y - Y10.x;
+    m.pxy = (Y11.y + Y11.x) + y11;
+    m.pxx = (Y20.y + Y20.x) + y20;
+    return m;
+}
+
 template <typename real>
 __device__ __forceinline__ Moments10<real> forward_moments(const real (&g)[3][3][3])
 {
@@ -160,6 +218,57 @@ __device__ __forceinline__ void back1d(real m0, real m1s, real m2s, real& fm, re
     fp = e + m1s;
     fm = e - m1s;
     f0 = fma(real(-2.0), e, m0);
+}
+
+// Eq.10, separable: r -> cz, then q -> cy, then p -> cx
+template <typename real>
+__device__ __forceinline__ void back_transform(const real (&Ms)[3][3][3], real (&g)[3][3][3])
+{
+    real A[3][3][3];   // [p][q][cz]
+#pragma unroll
+    for (int p = 0; p < 3; ++p)
+#pragma unroll
+        for (int q = 0; q < 3; ++q) back1d(Ms[p][q][0], Ms[p][q][1], Ms[p][q][2], A[p][q][0], A[p][q][1], A[p][q][2]);
+    real B[3][3][3];   // [p][cy][cz]
+#pragma unroll
+    for (int p = 0; p < 3; ++p)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) back1d(A[p][0][c], A[p][1][c], A[p][2][c], B[p][0][c], B[p][1][c], B[p][2][c]);
+#pragma unroll
+    for (int b = 0; b < 3; ++b)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) back1d(B[0][b][c], B[1][b][c], B[2][b][c], g[c][b][0], g[c][b][1], g[c][b][2]);
+}
+
+// fp32: the first two passes run on the pair (p = 1, p = 2), p = 0 on scalars; the last pass mixes p and stays scalar
+__device__ __forceinline__ void back1d2(float2 m0, float2 m1s, float2 m2s, float2& fm, float2& f0, float2& fp)
+{
+    const float2 e = fma2(make_float2(1.0f / 6.0f, 1.0f / 6.0f), m0, m2s);
+    fp = add2(e, m1s);
+    fm = sub2(e, m1s);
+    f0 = fma2(make_float2(-2.0f, -2.0f), e, m0);
+}
+__device__ __forceinline__ void back_transform(const float (&Ms)[3][3][3], float (&g)[3][3][3])
+{
+    float A0[3][3];     // [q][cz], p = 0
+    float2 A12[3][3];   // [q][cz], (p = 1, p = 2)
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+        back1d(Ms[0][q][0], Ms[0][q][1], Ms[0][q][2], A0[q][0], A0[q][1], A0[q][2]);
+        back1d2(make_float2(Ms[1][q][0], Ms[2][q][0]), make_float2(Ms[1][q][1], Ms[2][q][1]),
+                make_float2(Ms[1][q][2], Ms[2][q][2]), A12[q][0], A12[q][1], A12[q][2]);
+    }
+    float B0[3][3];     // [cy][cz]
+    float2 B12[3][3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        back1d(A0[0][c], A0[1][c], A0[2][c], B0[0][c], B0[1][c], B0[2][c]);
+        back1d2(A12[0][c], A12[1][c], A12[2][c], B12[0][c], B12[1][c], B12[2][c]);
+    }
+#pragma unroll
+    for (int b = 0; b < 3; ++b)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) back1d(B0[b][c], B12[b][c].x, B12[b][c].y, g[c][b][0], g[c][b][1], g[c][b][2]);
 }
 
 // In: g = pre-collision populations of the site.  Out: g = post-collision populations f*.
@@ -318,21 +427,7 @@ __device__ __forceinline__ void collide(real (&g)[3][3][3], const StepParams<rea
         }
     }
 
-    // Eq.10, separable: r -> cz, then q -> cy, then p -> cx
-    real A[3][3][3];   // [p][q][cz]
-#pragma unroll
-    for (int p = 0; p < 3; ++p)
-#pragma unroll
-        for (int q = 0; q < 3; ++q) back1d(Ms[p][q][0], Ms[p][q][1], Ms[p][q][2], A[p][q][0], A[p][q][1], A[p][q][2]);
-    real B[3][3][3];   // [p][cy][cz]
-#pragma unroll
-    for (int p = 0; p < 3; ++p)
-#pragma unroll
-        for (int c = 0; c < 3; ++c) back1d(A[p][0][c], A[p][1][c], A[p][2][c], B[p][0][c], B[p][1][c], B[p][2][c]);
-#pragma unroll
-    for (int b = 0; b < 3; ++b)
-#pragma unroll
-        for (int c = 0; c < 3; ++c) back1d(B[0][b][c], B[1][b][c], B[2][b][c], g[c][b][0], g[c][b][1], g[c][b][2]);
+    back_transform(Ms, g);
 }
 
 }  // namespace rflbm_dev
