@@ -278,9 +278,32 @@ step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const real* src, r
             if (PHASE == STEP_AA_ODD) {
                 // push to the neighbours x + c_q (slot q), misaligned by one element for cx = +-1: the partial
                 // sectors at the ends of a warp's 256 bytes are completed in L2 by the neighbouring warp's store
-                SiteIndex i;
-                i.x = x; i.y = y; i.z = z; i.zg = zg; i.valid = true; i.s = s; i.sl = 0; i.site = site;
-                scatter<real, WALLS, STEP_AA_ODD>(dst, G, i, g);
+                // Three per-thread column pointers (x-1, x, x+1 with the periodic wrap) plus a (row, slot) offset that is
+                // the same for the whole block: two address instructions per store, like the aligned stores below
+                // (the generic scatter() of rflbm_kernels.cuh rebuilds a 64-bit per-thread index for each of the 27).
+                const long long xm = (x == 0) ? G.nx - 1 : x - 1, xp = (x + 1 == G.nx) ? 0 : x + 1;
+                const unsigned long long col[3] = {reinterpret_cast<unsigned long long>(dst + xm),
+                                                   reinterpret_cast<unsigned long long>(dst + x),
+                                                   reinterpret_cast<unsigned long long>(dst + xp)};
+                const unsigned long long own = reinterpret_cast<unsigned long long>(dst + s);
+                const int yd[3] = {(y == 0) ? G.ny - 1 : y - 1, y, (y + 1 == G.ny) ? 0 : y + 1};
+                const int zd[3] = {(z == 0) ? G.nzs - 1 : z - 1, z, (z + 1 == G.nzs) ? 0 : z + 1};
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    // x + c_q is solid iff (cz=-1 and zg==1) or (cz=+1 and zg==nzg-2): back to the site itself as 26-q
+                    const bool bounce = WALLS && ((c == 0 && bounce_lo) || (c == 2 && bounce_hi));
+#pragma unroll
+                    for (int b = 0; b < 3; ++b) {
+                        const long long rowoff = (long long)G.px * yd[b] + G.pxy * zd[c];      // block-uniform
+#pragma unroll
+                        for (int a = 0; a < 3; ++a) {
+                            const int q = a + 3 * b + 9 * c;
+                            const unsigned long long push = col[a] + (unsigned long long)(((long long)q * G.QS + rowoff) * (long long)sizeof(real));
+                            const unsigned long long back = own + (unsigned long long)QS32 * ((unsigned)sizeof(real) * (26 - q));
+                            __stcs(reinterpret_cast<real*>((WALLS && bounce) ? back : push), g[c][b][a]);
+                        }
+                    }
+                }
             } else {
                 const unsigned long long out = reinterpret_cast<unsigned long long>(dst + s);
 #pragma unroll
