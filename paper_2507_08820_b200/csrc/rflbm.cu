@@ -14,20 +14,21 @@
 #include "rflbm_host.cuh"
 
 static size_t real_size(const rflbm* h) { return h->precision == RFLBM_F64 ? sizeof(double) : sizeof(float); }
-static size_t pop_bytes(const rflbm* h) { return (size_t)Q * (size_t)h->QS * real_size(h); }
+static size_t pop_elems(const rflbm* h);
+static size_t pop_bytes(const rflbm* h) { return pop_elems(h) * real_size(h); }
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 static constexpr size_t TABLE_BYTES = (LOG_TABLE_N + SC_TABLE_N) * sizeof(f64x2);
 enum { HALO_NONE = 0, HALO_FILL = 1, HALO_HOME = 2 };
 
-// Storage layout.  Population arrays are NOT packed back to back: for power-of-two lattices
-// N*sizeof(real) is a power of two and the 27 read streams + 27 write streams of a step would all hit the same DRAM
-// channel/bank residues.  A pad of 37 x 256 B skews successive arrays; small lattices only round up to 32.
+// Storage layout: P[z][y][q][x], i.e. the 27 populations of one lattice ROW are 27 consecutive
+// padded rows of px elements: slot stride QS = px, row stride 27 px, layer stride 27 px ny.  Everything a block touches
+// in one row step (27 rows written, 9 source rows of 3 populations each read) then lies in a few contiguous pieces of
+// 12-110 KB instead of 54 streams a gigabyte apart.
 static void set_layout(rflbm* h)
 {
-    const long long ns = (long long)h->px * h->ny * (h->nz + (h->slab ? 2 : 0));
-    const long long pad = (ns >= (1 << 16)) ? 37 * 32 : 0;
-    h->QS = (ns + 31) / 32 * 32 + pad;
+    h->QS = h->px;
 }
+static size_t pop_elems(const rflbm* h) { return (size_t)Q * (size_t)h->px * (size_t)h->ny * (size_t)(h->nz + (h->slab ? 2 : 0)); }
 
 // launch grid of the one-thread-per-site kernels over the owned layers [zc, zc+zn) of the next launch
 static dim3 zgrid(const rflbm* h) { return dim3(h->grid.x, h->grid.y, (unsigned)h->zn); }
@@ -61,7 +62,7 @@ typedef CUresult (*encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_
                                     const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                     CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-// 4-D view [27][nzs][ny][nx] (row pitch px) of one population buffer, box = BOX_X consecutive x of one row of BOX_Q arrays
+// 4-D view [nzs][ny][27][nx] (x pitch px) of one population buffer, box = BOX_X consecutive x of BOX_Q populations of one row
 static bool make_tensor_map(rflbm* h, void* base, CUtensorMap* out)
 {
     void* fn = nullptr;
@@ -73,9 +74,10 @@ static bool make_tensor_map(rflbm* h, void* base, CUtensorMap* out)
     }
     const bool f64 = h->precision == RFLBM_F64;
     const cuuint64_t es = f64 ? 8 : 4;
-    const cuuint64_t dims[4] = {(cuuint64_t)h->nx, (cuuint64_t)h->ny, (cuuint64_t)(h->nz + (h->slab ? 2 : 0)), (cuuint64_t)Q};
-    const cuuint64_t strides[3] = {(cuuint64_t)h->px * es, (cuuint64_t)h->px * h->ny * es, (cuuint64_t)h->QS * es};
-    const cuuint32_t box[4] = {(cuuint32_t)(h->tma_tx + 2 * (16 / (int)es)), 1, 1, BOX_Q};     // 16-byte aligned starts
+    // dimensions (x, q, y, z): strides px, 27 px, 27 px ny elements (each a multiple of the one before)
+    const cuuint64_t dims[4] = {(cuuint64_t)h->nx, (cuuint64_t)Q, (cuuint64_t)h->ny, (cuuint64_t)(h->nz + (h->slab ? 2 : 0))};
+    const cuuint64_t strides[3] = {(cuuint64_t)h->px * es, (cuuint64_t)Q * h->px * es, (cuuint64_t)Q * h->px * h->ny * es};
+    const cuuint32_t box[4] = {(cuuint32_t)(h->tma_tx + 2 * (16 / (int)es)), BOX_Q, 1, 1};     // 16-byte aligned starts
     const cuuint32_t estr[4] = {1, 1, 1, 1};
     const CUresult r = ((encode_tiled_fn)fn)(out, f64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, base, dims, strides, box, estr,
                                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,

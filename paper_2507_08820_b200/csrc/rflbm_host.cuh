@@ -60,9 +60,9 @@ inline Geom make_geom(const rflbm* h)
     G.zc = h->zc;
     G.zg0 = h->slab ? h->z0 - 1 : 0;
     G.nzg = h->slab ? h->nzg : h->nz;
-    G.px = h->px;
-    G.pxy = (long long)h->px * h->ny;
-    G.QS = h->QS;
+    G.px = Q * h->px;                              // P[z][y][q][x]: consecutive rows of one population are 27 px apart
+    G.pxy = (long long)Q * h->px * h->ny;
+    G.QS = h->px;
     G.N = h->N;
     return G;
 }

@@ -78,7 +78,7 @@ __device__ __forceinline__ void tma_load_box(uint32_t dst, const CUtensorMap* tm
 {
     asm volatile(
         "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
-        ::"r"(dst), "l"((unsigned long long)tmap), "r"(x), "r"(y), "r"(z), "r"(q), "r"(bar)
+        ::"r"(dst), "l"((unsigned long long)tmap), "r"(x), "r"(q), "r"(y), "r"(z), "r"(bar)      // tensor map dimensions: (x, q, y, z)
         : "memory");
 }
 
