@@ -45,9 +45,9 @@ enum { RFLBM_OK = 0, RFLBM_EINVAL = -1, RFLBM_ESTATE = -2, RFLBM_ENOMEM = -3, RF
 int rflbm_create(int nx, int ny, int nz, double tau, double kT, double rho0, uint64_t seed, int precision,
                  rflbm_t** out);
 
-/* Bytes of device workspace the handle needs: two population buffers 2*27*QS*sizeof(real) (A-B scheme; one for AA;
- * QS = storage sites px*ny*nzs rounded up to 32 plus a 9.5 KB skew when >= 65536, px = nx rounded up to whole 128-byte
- * lines for nx >= 32, nzs = nz, or nz+2 in slab mode) plus a 4 KiB reduction scratch and 12 KiB of Box-Muller tables. */
+/* Bytes of device workspace the handle needs: two population buffers of 27*px*ny*nzs*sizeof(real) bytes each (A-B
+ * scheme; one for AA; px = nx rounded up to whole 128-byte lines for nx >= 32, nzs = nz, or nz+2 in slab mode), each
+ * rounded up to 256 bytes, plus a 4 KiB reduction scratch and 12 KiB of Box-Muller tables. */
 size_t rflbm_workspace_bytes(const rflbm_t* h);
 
 /* Borrow `bytes` of device memory at dev_ptr (256-byte aligned) as the workspace.

@@ -46,9 +46,9 @@ struct Geom {
     int zc;                 // first owned layer this LAUNCH works on (0 unless rflbm_run_host pipelines z-chunks), grid.z counts from it
     int zg0;                // global z of storage layer 0: 0, or z0 - 1 in slab mode
     int nzg;                // global number of layers (= nz without a slab)
-    int px;                 // row pitch of the internal buffers, in elements
-    long long pxy;          // px * ny
-    long long QS;           // elements between consecutive population arrays inside a buffer
+    int px;                 // elements between consecutive y rows of one population (27 x the padded row length)
+    long long pxy;          // px * ny: elements between consecutive z layers
+    long long QS;           // elements between consecutive populations of one site (the padded row length)
     long long N;            // nx * ny * nz: length of the canonical (boundary) arrays
 };
 

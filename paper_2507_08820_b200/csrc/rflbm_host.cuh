@@ -16,7 +16,7 @@ struct rflbm {
     int px;              // row pitch of the internal buffers (elements): nx rounded up so that rows are 16-byte aligned
     int slab;            // 1 after rflbm_set_slab: ghost layers below and above, global z for walls and the RNG key
     int z0, nzg;         // slab: global z of the first owned layer, global number of layers
-    long long QS;        // elements between population arrays inside a buffer: storage sites rounded up to 32 plus padding
+    long long QS;        // slot stride of the internal buffers = px (layout P[z][y][q][x])
     double tau, kT, rho0;
     uint64_t seed;
     int precision;

@@ -1,7 +1,8 @@
 // rflbm_kernels.cuh — CUDA kernels of the Reg-FLBM path (sm_100a).
 //
-// Storage: SoA buffers P[q][z][y][x] of `real` in the lex order of rflbm_lattice.cuh, rows
-// px >= nx elements apart (16-byte aligned rows whatever nx is), the 27 arrays QS elements apart.
+// Storage: buffers P[z][y][q][x] of `real`, q in the lex order of rflbm_lattice.cuh: slot stride
+// Geom::QS (= the padded row length >= nx, 16-byte aligned rows whatever nx is), row stride Geom::px = 27 QS, layer
+// stride Geom::pxy.  The kernels only ever use these three strides.
 //   A-B scheme: two buffers holding POST-collision, UN-streamed populations (R10).  A step PULLS
 //     S_t[q](x) = P_{t-1}[q](x - c_q)  (Eq.7 :87; bounce-back: P_{t-1}[26-q](x) when x - c_q is solid, R12),
 //     collides in registers and stores P_t[q](x): 27 neighbour reads (coalesced, at most one element off alignment)
