@@ -103,12 +103,6 @@ __device__ __forceinline__ float2 sub2(float2 a, float2 b)
     asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(f2_bits(a)), "l"(f2_bits(b)));
     return f2_from(d);
 }
-__device__ __forceinline__ float2 mul2(float2 a, float2 b)
-{
-    unsigned long long d;
-    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(f2_bits(a)), "l"(f2_bits(b)));
-    return f2_from(d);
-}
 __device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c)
 {
     unsigned long long d;
@@ -277,45 +271,6 @@ __device__ __forceinline__ void back_transform(const float (&Ms)[3][3][3], float
         for (int c = 0; c < 3; ++c) back1d(B0[b][c], B12[b][c].x, B12[b][c].y, g[c][b][0], g[c][b][1], g[c][b][2]);
 }
 
-// The two Box-Muller pairs of one Philox call (words 0,1 and 2,3): radius and (sin, cos) of each.
-__device__ __forceinline__ void normal_polar_call(const uint32_t (&w)[4], const f64x2* lg, const f64x2* sc, double (&R)[2],
-                                                  double (&sn)[2], double (&cs)[2])
-{
-    normal_polar(w[0], w[1], lg, sc, R[0], sn[0], cs[0]);
-    normal_polar(w[2], w[3], lg, sc, R[1], sn[1], cs[1]);
-}
-// fp32 (R14, rflbm_rng.cuh): the same operations as two calls of normal_polar(float), the three multiply-adds that both
-// pairs share done on packed pairs (uniform of the radius, -2 ln2 lg2, angle)
-__device__ __forceinline__ void normal_polar_call(const uint32_t (&w)[4], const f64x2*, const f64x2*, float (&R)[2],
-                                                  float (&sn)[2], float (&cs)[2])
-{
-    const uint32_t k0 = w[0] >> 8, k1 = w[2] >> 8;
-    const float2 ua = fma2(make_float2((float)k0, (float)k1), make_float2(1.0f / 16777216.0f, 1.0f / 16777216.0f),
-                           make_float2(1.0f / 33554432.0f, 1.0f / 33554432.0f));
-    float2 l2;
-    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(l2.x) : "f"(ua.x));
-    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(l2.y) : "f"(ua.y));
-    float2 W = mul2(l2, make_float2(-1.3862943611198906f, -1.3862943611198906f));
-    if (k0 >= 16777216u - 16384u) {                                 // u within 2^-10 of 1: the series (rflbm_rng.cuh)
-        const float v = ((float)(16777216u - k0) - 0.5f) * (1.0f / 16777216.0f);
-        W.x = fmaf(v, v, 2.0f * v);
-    }
-    if (k1 >= 16777216u - 16384u) {
-        const float v = ((float)(16777216u - k1) - 0.5f) * (1.0f / 16777216.0f);
-        W.y = fmaf(v, v, 2.0f * v);
-    }
-    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(R[0]) : "f"(W.x));
-    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(R[1]) : "f"(W.y));
-    constexpr float TWO_PI_24 = 6.283185307179586f / 16777216.0f;
-    const float2 th = fma2(make_float2((float)((int)(w[1] >> 8) - 8388608), (float)((int)(w[3] >> 8) - 8388608)),
-                           make_float2(TWO_PI_24, TWO_PI_24), make_float2(0.5f * TWO_PI_24, 0.5f * TWO_PI_24));
-    float s, c;
-    __sincosf(th.x, &s, &c);
-    sn[0] = -s; cs[0] = -c;
-    __sincosf(th.y, &s, &c);
-    sn[1] = -s; cs[1] = -c;
-}
-
 // In: g = pre-collision populations of the site.  Out: g = post-collision populations f*.
 // BGK = false: Reg-FLBM, Eq.24 (the hot path).  BGK = true: BGK-FLBM, Eq.11 (:109-111), the paper's comparison
 // model: every non-conserved mode relaxes at the one rate omega, M_k = M_k^eq + (1-omega)(m_k - M_k^eq), which
@@ -454,11 +409,10 @@ __device__ __forceinline__ void collide(real (&g)[3][3][3], const StepParams<rea
         for (int call = 0; call < 6; ++call) {
             uint32_t w[4];
             philox_call(ps, P.rng, call, w);
-            real Rh[2], snh[2], csh[2];
-            normal_polar_call(w, lg, sc, Rh, snh, csh);        // the two Box-Muller pairs of this call
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
-                const real R = Rh[h], sn = snh[h], cs = csh[h];
+                real R, sn, cs;
+                normal_polar(w[2 * h], w[2 * h + 1], lg, sc, R, sn, cs);
                 const int k = 4 + 4 * call + 2 * h;            // modes k (first normal R cs) and k+1 (second, R sn), R8
                 const int ca = amp_class(mode_p(k), mode_q(k), mode_r(k));
                 real& m0 = Ms[mode_p(k)][mode_q(k)][mode_r(k)];
