@@ -63,7 +63,7 @@ typedef CUresult (*encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_
                                     CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 // 4-D view [nzs][ny][27][nx] (x pitch px) of one population buffer, box = BOX_X consecutive x of BOX_Q populations of one row
-static bool make_tensor_map(rflbm* h, void* base, CUtensorMap* out)
+static bool make_tensor_map(rflbm* h, void* base, CUtensorMap* out, bool store_box = false)
 {
     void* fn = nullptr;
     cudaDriverEntryPointQueryResult qres;
@@ -77,7 +77,7 @@ static bool make_tensor_map(rflbm* h, void* base, CUtensorMap* out)
     // dimensions (x, q, y, z): strides px, 27 px, 27 px ny elements (each a multiple of the one before)
     const cuuint64_t dims[4] = {(cuuint64_t)h->nx, (cuuint64_t)Q, (cuuint64_t)h->ny, (cuuint64_t)(h->nz + (h->slab ? 2 : 0))};
     const cuuint64_t strides[3] = {(cuuint64_t)h->px * es, (cuuint64_t)Q * h->px * es, (cuuint64_t)Q * h->px * h->ny * es};
-    const cuuint32_t box[4] = {(cuuint32_t)(h->tma_tx + 2 * (16 / (int)es)), BOX_Q, 1, 1};     // 16-byte aligned starts
+    const cuuint32_t box[4] = {store_box ? 32u : (cuuint32_t)(h->tma_tx + 2 * (16 / (int)es)), store_box ? (cuuint32_t)Q : (cuuint32_t)BOX_Q, 1, 1};     // 16-byte aligned starts
     const cuuint32_t estr[4] = {1, 1, 1, 1};
     const CUresult r = ((encode_tiled_fn)fn)(out, f64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, base, dims, strides, box, estr,
                                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
@@ -174,7 +174,8 @@ extern "C" int rflbm_set_workspace(rflbm_t* h, void* dev_ptr, size_t bytes)
     // TMA path: every lattice with nx >= 32 (rows of the internal buffers are 16-byte aligned by construction)
     h->tma_ok = false;
     if (h->tma_tx != 0)
-        h->tma_ok = make_tensor_map(h, h->buf[0], &h->tmap[0]) && (nbuf == 1 || make_tensor_map(h, h->buf[1], &h->tmap[1]));
+        h->tma_ok = make_tensor_map(h, h->buf[0], &h->tmap[0]) && (nbuf == 1 || make_tensor_map(h, h->buf[1], &h->tmap[1])) &&
+                    make_tensor_map(h, h->buf[0], &h->tmap_out[0], true) && (nbuf == 1 || make_tensor_map(h, h->buf[1], &h->tmap_out[1], true));
     return RFLBM_OK;
 }
 

@@ -40,7 +40,8 @@ struct rflbm {
     uint64_t launches;
     cudaStream_t stream;
     dim3 block, grid;
-    CUtensorMap tmap[2];  // TMA descriptors of the two population buffers
+    CUtensorMap tmap[2];  // TMA descriptors of the two population buffers (load boxes: TX + halo, 3 populations)
+    CUtensorMap tmap_out[2];  // the same buffers with the store box of one warp: 32 x, all 27 populations of one row
     bool tma_ok;
     int tma_tx;           // tile width of the TMA kernel for this lattice: 128, 64 or 32 (0: nx < 32, plain kernel only)
     int variant;          // RFLBM_KERNEL_AUTO / _PLAIN / _TMA
@@ -76,8 +77,10 @@ static inline void launch_one(rflbm* h, const StepParams<real>& P)
     real* dst = (real*)h->buf[PHASE == STEP_AB ? (h->cur ^ 1) : h->cur];
     if constexpr (TX != 0) {
         const dim3 grid((h->nx + TX - 1) / TX, (h->ny + h->tma_rows - 1) / h->tma_rows, h->zn);
-        step_kernel_tma<real, TX, WALLS, FORCE, NOISE, BGK, GHOST, PHASE><<<grid, BLOCK_T, 0, h->stream>>>(
-            h->tmap[h->cur], src, dst, P, h->tma_rows);
+        auto kern = step_kernel_tma<real, TX, WALLS, FORCE, NOISE, BGK, GHOST, PHASE>;
+        constexpr int dyn = tma_store_bytes<real, PHASE>();       // per-warp output boxes of the TMA-store instantiations
+        kern<<<grid, BLOCK_T, dyn, h->stream>>>(h->tmap[h->cur], h->tmap_out[PHASE == STEP_AB ? (h->cur ^ 1) : h->cur], src, dst, P,
+                                                 h->tma_rows);
     } else {
         const dim3 grid(h->grid.x, h->grid.y, h->zn);
         step_kernel<real, WALLS, FORCE, NOISE, BGK, GHOST, PHASE><<<grid, h->block, 0, h->stream>>>(src, dst, P);

@@ -82,6 +82,17 @@ __device__ __forceinline__ void tma_load_box(uint32_t dst, const CUtensorMap* tm
         : "memory");
 }
 
+// store of one box from shared memory (bulk async-group completion); same coordinate order as the loads
+__device__ __forceinline__ void tma_store_box(const CUtensorMap* tmap, uint32_t src, int x, int y, int z, int q)
+{
+    asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.bulk_group [%0, {%1, %2, %3, %4}], [%5];"
+                 ::"l"((unsigned long long)tmap), "r"(x), "r"(q), "r"(y), "r"(z), "r"(src)
+                 : "memory");
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+}
+__device__ __forceinline__ void tma_store_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
 __device__ __forceinline__ bool elect_one()
 {
     uint32_t pred;
@@ -134,22 +145,39 @@ __device__ __forceinline__ void issue_tile(const CUtensorMap* tmap, uint32_t s_i
             issue_row<real, TX, WALLS, PHASE>(tmap, s_in + (uint32_t)(r * 9 * T::BOX_PITCH_BYTES), bar, x0, yb + r, z, zg, G);
 }
 
+// Which instantiations write their results with bulk tensor STORES (SASS UTMASTG): each warp stages its 32 sites x 27
+// populations in shared memory ([27][32], conflict-free STS.[tid*size + immediate]) and lane 0 issues ONE
+// cp.async.bulk.tensor store of the box (32 x, 27 q, 1 y, 1 z) — in the layout P[z][y][q][x] the 27 rows a lattice row
+// writes are consecutive, so one box replaces 27 STG and their 54 address instructions per warp.  No block barrier: a
+// warp waits only for its own previous box to have been read (cp.async.bulk.wait_group.read) before it refills it.
+// Measured in one call each, sustained, 512^3 (profiles/r02_variants.md): fp32 A-B 5.177 -> 5.044 and 5.491 -> 5.300 ms
+// (-2.6 / -3.5 %, the fp32 kernel is issue bound; 6 blocks of 79 registers instead of 8 of 64: the box stage makes it 7
+// by shared memory anyway); fp64 A-B 9.639 -> 9.658 and 10.272 -> 10.291 ms (+0.2 %: 39 fewer instructions per 32 sites
+// and a slightly higher clock under the power cap, but the fence + warp sync at the end of every row is exposed with 3
+// warps per scheduler), so fp64 keeps its per-thread streaming stores.  Issuing the box one row late, behind the next
+// block barrier: fp64 +2 %, fp32 +0.6 % slower than the immediate form.  The odd AA phase cannot use a box at all (its
+// cx = +-1 populations move by one element: box starts must be multiples of 16 bytes).
+template <typename real, int PHASE> __host__ __device__ constexpr bool tma_store() { return sizeof(real) == 4 && PHASE != STEP_AA_ODD; }
+template <typename real, int PHASE> __host__ __device__ constexpr int tma_store_bytes()
+{
+    return tma_store<real, PHASE>() ? (BLOCK_T / 32) * Q * 32 * (int)sizeof(real) : 0;
+}
+
 // fp64, A-B scheme: 3 blocks per SM (up to 168 registers; 41 KB each).  Measured against 4 blocks of 128 registers in
 // one call, sustained: 9.73 vs 9.80 and 9.86 vs 9.92 ms (24 fewer instructions per site, no spills; 5 blocks of 96
 // registers: 10.13).  The in-place phases keep 4 blocks (10.09 vs 10.14 with 3).  fp32: 64 registers, 15 KB -> 8 blocks.
 template <typename real, int TX, bool WALLS, bool FORCE, bool NOISE, bool BGK, bool GHOST, int PHASE>
-__global__ void __launch_bounds__(BLOCK_T, sizeof(real) == 8 ? (PHASE == STEP_AB ? 3 : 4) : 8)
-step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const real* src, real* dst,
+__global__ void __launch_bounds__(BLOCK_T, sizeof(real) == 8 ? (PHASE == STEP_AB ? 3 : 4) : (tma_store<real, PHASE>() ? 6 : 8))
+step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const __grid_constant__ CUtensorMap tmap_dst, const real* src, real* dst,
                 const __grid_constant__ StepParams<real> P, int rows)
 {
+    constexpr bool TSTORE = tma_store<real, PHASE>();
+    extern __shared__ __align__(128) unsigned char s_dyn[];    // TSTORE: one [27][32] output box per warp
     using T = TmaGeom<real, TX>;
     constexpr bool TABLES = NOISE && sizeof(real) == 8;         // the fp32 Box-Muller needs no tables
     __shared__ __align__(128) real s_stage[T::STAGE_BYTES / sizeof(real)];
     __shared__ f64x2 s_tab[TABLES ? LOG_TABLE_N + SC_TABLE_N : 1];
     __shared__ __align__(8) unsigned long long s_bar;
-#ifdef RFLBM_EXP_NOSYNC
-    __shared__ __align__(8) unsigned long long s_empty;      // consumer release: one arrival per warp
-#endif
 
     const Geom& G = P.G;
     const int z = (int)blockIdx.z + G.zc + G.z_lo, zg = z + G.zg0;
@@ -163,14 +191,8 @@ step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const real* src, r
     const int y_end = min(y_begin + rows, G.ny);
     const uint32_t bar = smem_u32(&s_bar), in0 = smem_u32(&s_stage[0]);
 
-#ifdef RFLBM_EXP_NOSYNC
-    const uint32_t empty = smem_u32(&s_empty);
-#endif
     if (warp == 0 && elect_one()) {
         mbar_init(bar, 1);
-#ifdef RFLBM_EXP_NOSYNC
-        mbar_init(empty, BLOCK_T / 32);
-#endif
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         issue_tile<real, TX, WALLS, PHASE>(&tmap_src, in0, bar, x0, y_begin, y_end, z, zg, G);
     }
@@ -185,6 +207,9 @@ step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const real* src, r
     const real* tile = &s_stage[0] + r * T::ROW_STAGE + xl;
     const bool bounce_lo = WALLS && zg == 1, bounce_hi = WALLS && zg == G.nzg - 2;
     uint32_t parity = 0;
+    const int lane = tid & 31;
+    real* const s_out = reinterpret_cast<real*>(s_dyn) + (size_t)(tid >> 5) * (Q * 32) + lane;     // this thread's column of its warp's box
+    const uint32_t out_box = smem_u32(reinterpret_cast<real*>(s_dyn) + (size_t)warp * (Q * 32));
     // row-invariant parts of the storage index and of the Philox site key (the key is < 2^32: 32-bit arithmetic is exact)
     const long long s_col = (long long)x + G.pxy * z;
     const uint32_t site_col = (uint32_t)x + (uint32_t)G.nx * (uint32_t)G.ny * (uint32_t)zg;
@@ -244,19 +269,9 @@ step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const real* src, r
                 }
             }
         }
-#ifdef RFLBM_EXP_NOSYNC
-        // the tile is in registers: every warp releases the stage; only the issuing lane waits for all four
-        __syncwarp();
-        if (elect_one()) mbar_arrive(empty);
-        if (warp == 0 && yb + T::RB < y_end && elect_one()) {
-            mbar_wait(empty, parity ^ 1u);
-            issue_tile<real, TX, WALLS, PHASE>(&tmap_src, in0, bar, x0, yb + T::RB, y_end, z, zg, G);
-        }
-#else
         __syncthreads();                                       // the tile is in registers: the stage is free
         if (warp == 0 && yb + T::RB < y_end && elect_one())
             issue_tile<real, TX, WALLS, PHASE>(&tmap_src, in0, bar, x0, yb + T::RB, y_end, z, zg, G);
-#endif
 
         if (PHASE != STEP_AA_EVEN && edge_warp && row_ok) {
             if (wrap_lo || wrap_hi) {
@@ -272,7 +287,7 @@ step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const real* src, r
                 }
             }
         }
-        if (active && row_ok) {
+        if ((TSTORE ? __any_sync(0xffffffffu, active) : active) && row_ok) {       // TSTORE: whole warps (lanes beyond nx are clipped by the store)
             const uint32_t site = site_col + (uint32_t)G.nx * (uint32_t)y;
             collide<real, FORCE, NOISE, BGK, GHOST>(g, P, site, s_tab, s_tab + LOG_TABLE_N);
             if (PHASE == STEP_AA_ODD) {
@@ -304,6 +319,22 @@ step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const real* src, r
                         }
                     }
                 }
+            } else if (TSTORE) {
+                // all stores of the warp as ONE bulk tensor store: the 27 rows of a lattice row are consecutive in P[z][y][q][x]
+                if (lane == 0) tma_store_wait_read();           // the previous box has been read out of shared memory
+                __syncwarp();
+#pragma unroll
+                for (int c = 0; c < 3; ++c)
+#pragma unroll
+                    for (int b = 0; b < 3; ++b)
+#pragma unroll
+                        for (int a = 0; a < 3; ++a) {
+                            const int q = a + 3 * b + 9 * c;
+                            s_out[((PHASE == STEP_AA_EVEN) ? 26 - q : q) * 32] = g[c][b][a];
+                        }
+                fence_proxy_async();                            // generic-proxy writes -> visible to the async proxy
+                __syncwarp();
+                if (lane == 0) tma_store_box(&tmap_dst, out_box, x, y, z, 0);     // lanes beyond nx are clipped by the tensor map
             } else {
                 const unsigned long long out = reinterpret_cast<unsigned long long>(dst + s);
 #pragma unroll
@@ -322,6 +353,7 @@ step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const real* src, r
             }
         }
     }
+    if (TSTORE && lane == 0) tma_store_wait_read();             // shared memory stays valid until the last box has been read
 }
 
 }  // namespace rflbm_dev
