@@ -51,6 +51,9 @@ def parse_args():
     p.add_argument("--variant", default="auto", choices=["auto", "plain", "tma"])
     p.add_argument("--model", default="reg", choices=["reg", "bgk"])
     p.add_argument("--scheme", default="ab", choices=["ab", "aa"])
+    p.add_argument("--decomp", default="replicas", choices=["replicas", "slab"],
+                   help="N > 1: independent replicas (BASELINE.json: no sharding), or z slabs of ONE lattice of N times the "
+                        "height with the faces exchanged every step (paper_2507_08820_b200/slab.py; PAPER.md:292, :300)")
     p.add_argument("--no-e2e", action="store_true")
     p.add_argument("--no-sustained", action="store_true")
     p.add_argument("--e2e-serial", action="store_true")
@@ -236,13 +239,26 @@ def run_ours(args):
     N = nx * ny * nz
     K, W = args.steps, max(3, args.warmup)
 
-    sim = binding.Rflbm(nx, ny, nz, WORKLOAD["tau"], args.kT, WORKLOAD["rho0"], WORKLOAD["seed"], prec, device=dev,
-                        scheme=binding.SCHEME_AA if args.scheme == "aa" else binding.SCHEME_AB)
+    scheme = binding.SCHEME_AA if args.scheme == "aa" else binding.SCHEME_AB
+    lat = None
+    if args.decomp == "slab":                       # one lattice nx x ny x (nz * world): every rank owns nz layers of it
+        from paper_2507_08820_b200 import slab
+        lat = slab.SlabLattice(nx, ny, nz * world, WORKLOAD["tau"], args.kT, WORKLOAD["rho0"], WORKLOAD["seed"], prec,
+                               device=dev, scheme=scheme)
+        sim, step = lat.sim, lat.step
+        args.no_e2e = True                          # rflbm_run_host is the single-handle job
+    else:
+        sim = binding.Rflbm(nx, ny, nz, WORKLOAD["tau"], args.kT, WORKLOAD["rho0"], WORKLOAD["seed"], prec, device=dev,
+                            scheme=scheme)
+        step = sim.step
     sim.set_kernel_variant({"auto": binding.KERNEL_AUTO, "plain": binding.KERNEL_PLAIN, "tma": binding.KERNEL_TMA}[args.variant])
     if args.model == "bgk":
         sim.set_model(binding.MODEL_BGK)
-    sim.init()
-    sim.step(W)                                     # warm-up: also thermalises the state
+    if lat is not None:
+        lat.init()
+    else:
+        sim.init()
+    step(W)                                         # warm-up: also thermalises the state
     torch.cuda.synchronize(dev)
 
     # ---- device-resident timing: K launches of the step kernel, CUDA events on the launching stream
@@ -258,7 +274,7 @@ def run_ours(args):
         if rank == 0:
             sampler.start()
         ev0.record(stream)
-        sim.step(nsteps)
+        step(nsteps)
         ev1.record(stream)
         torch.cuda.synchronize(dev); barrier_all()
         clk = sampler.stop() if rank == 0 else None
@@ -352,7 +368,10 @@ def run_ours(args):
                                   else f"; in-place AA buffer {27 * es * N / 1e9:.1f} GB"),
                    "scheme": args.scheme, "model": args.model, "kernel_variant": args.variant,
                    "l2": "no flush needed: each step streams 2*27*N*sizeof(real) bytes >> 126 MB L2",
-                   "parallelism": "replicas only" if world > 1 else "single GPU"},
+                   "parallelism": ("single GPU" if world == 1 else "replicas only") if lat is None else
+                                  f"z slabs: ONE {nx}x{ny}x{nz * world} lattice, {nz} layers per rank, 2 faces of "
+                                  f"{lat.face_bytes / 1e6:.1f} MB per rank and step ({lat.transport.backend} send/recv; "
+                                  "one rank: device-to-device through the pack/unpack kernels)"},
         "clocks": clocks, "sustained": sustained, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
         "cpu_baseline": cpu, "hbm_gbs": achieved, "mass_rel_err": mass_err,
     }
