@@ -313,7 +313,7 @@ def run_ours(args):
         u_o = torch.empty((3,) + shape, dtype=dt).pin_memory()
         scratch = torch.empty(4 * N * es, dtype=torch.uint8, device=dev)
         copy_stream = torch.cuda.Stream(device=dev)
-        sim.set_copy_stream(None if args.e2e_serial else copy_stream)  # pipelined over z chunks unless --e2e-serial
+        sim.set_copy_stream(None if args.e2e_serial else copy_stream)  # pipelined (time-skewed along z) unless --e2e-serial
         sim.run_host(rho_h, u_h, 2, rho_o, u_o, scratch)              # warm the copy path
         barrier_all(); torch.cuda.synchronize(dev)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -326,7 +326,7 @@ def run_ours(args):
                "h2d_bytes_per_step": 4 * N * es / K, "d2h_bytes_per_step": 4 * N * es / K,
                "ms_total": ms_e, "pipelined": not args.e2e_serial,
                "what": "rflbm_run_host: pinned host rho,u -> device, init, K steps, moments, device -> pinned host, "
-                       "sync; bytes are per job / K; copies on a second stream, z-chunked and overlapped with the "
+                       "sync; bytes are per job / K; copies on a second stream in bands of z layers, the steps time-skewed behind the upload front, the download behind the last step: all overlapped with the "
                        "kernels (include/rflbm.h)" if not args.e2e_serial else
                        "rflbm_run_host, serial form: pinned host rho,u -> device, init, K steps, moments, device -> "
                        "pinned host, sync; bytes are per job / K"}

@@ -169,12 +169,15 @@ int rflbm_debug_rng(rflbm_t* h, uint64_t step, void* words_dev, void* normals_de
  * back to rho_out_host / u_out_host and synchronise.  scratch_dev: caller-owned device buffer of at least
  * 4*N*sizeof(real) bytes.  rho_host = u_host = NULL -> uniform rho0, u=0 start (no upload).
  * Afterwards the handle is in the state rflbm_init + rflbm_step(nsteps) leaves it in.
- * With a copy stream (rflbm_set_copy_stream) and the A-B scheme the job is PIPELINED over up to 32 chunks of z layers:
- * a chunk is initialised as soon as it and its two neighbours have been uploaded, a chunk that has done L steps takes
- * step L+1 as soon as both neighbours have done L (the steps run behind the upload front), and the moments of a chunk
- * that has finished are downloaded while the others are still stepping.  Every launch is the same kernel restricted to
- * a z range, so the results are bit-identical to the serial form.  Without a copy stream, in the AA scheme, or with
- * nz < 3, everything runs one after the other on the handle's stream.  ESTATE in slab mode. */
+ * With a copy stream (rflbm_set_copy_stream) and the A-B scheme the job is PIPELINED, time-skewed along z: the fields are
+ * uploaded in up to 32 bands of consecutive layers; as soon as the layers [0, U) are on the device, the state after L steps
+ * is completed on the layers [L+1, U-1-L) for EVERY L (a step reaches one layer up and down, so each level runs one layer
+ * behind the level below it), and the moments of the layers that have reached step nsteps are downloaded while the rest
+ * is still being uploaded or stepped; the triangular seam the periodic ring leaves open is closed at the end.  Jobs of
+ * more than 24 steps skew only the first and the last 12 steps and run the steps in between as whole-lattice launches.
+ * Every launch is the same kernel restricted to a z range, so the results are bit-identical to the serial form.
+ * Without a copy stream, in the AA scheme, or with nz < 3, everything runs one after the other on the handle's stream.
+ * ESTATE in slab mode. */
 int rflbm_run_host(rflbm_t* h, const void* rho_host, const void* u_host, int nsteps, void* rho_out_host,
                    void* u_out_host, void* scratch_dev, size_t scratch_bytes);
 

@@ -234,7 +234,7 @@ class Rflbm:
 
     def run_host(self, rho_host, u_host, nsteps, rho_out_host, u_out_host, scratch=None):
         """End-to-end job on HOST tensors (pinned for speed): upload, init, step, moments, download, sync;
-        pipelined over z chunks when a copy stream has been set (include/rflbm.h)."""
+        pipelined (time-skewed along z) when a copy stream has been set (include/rflbm.h)."""
         t = self.torch
         es = 8 if self.precision == F64 else 4
         with self._ctx():

@@ -4,6 +4,7 @@
 // The library never allocates device memory and never creates a stream (include/rflbm.h).
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -563,65 +564,63 @@ static int run_host_serial(rflbm* h, const void* rho_host, const void* u_host, i
     return check_cuda(h, cudaStreamSynchronize(h->stream), "cudaStreamSynchronize");
 }
 
-// Pipelined form (A-B scheme, a copy stream given): the lattice is cut into C chunks of consecutive z layers.  The
-// copies run on the copy stream, the kernels on the handle's stream, ordered by events:
-//   * chunk c of (rho, u) is uploaded, and as soon as chunks c-1, c, c+1 are on the device chunk c is initialised;
-//   * a chunk that has done L steps may do step L+1 once both neighbours have done at least L (the pull reads one
-//     layer of each neighbour; the A-B buffer that step L+1 overwrites held level L-1, which nobody needs any more):
-//     the steps start behind the upload front and form a pyramid in (z, t) while the rest is still on the wire;
-//   * at the end the chunks are brought to step K one after the other (each needs a cone of its neighbours), and the
-//     moments of a finished chunk are computed and downloaded while the others are still stepping.
-// Every launch is the same kernel restricted to a z range (Geom::zc), so the result is bit-identical to the serial form.
+// Pipelined form (A-B scheme, a copy stream given): time-skewed along z.  The copies run on the copy stream, the kernels
+// on the handle's stream, ordered by events.  Call "level L" the state after L steps (level 0: initialised; level L of
+// layer z lives in buffer L & 1).  Bringing layers [a, b) to level L reads level L-1 on [a-1, b+1) — the pull reaches one
+// layer up and down — and overwrites level L-2 there, which nobody needs once level L-1 is complete on [a-1, b+1).  So as
+// soon as the layers [0, U) of (rho, u) are on the device, level L can be completed on [L+1, U-1-L): every band of CH
+// uploaded layers lets EVERY level advance by CH layers, each one layer behind the level below it (a parallelogram in
+// (z, t)), and the moments of the layers that have reached the last level go back to the host while the rest is still
+// on the wire or stepping.  The ring is periodic, so one triangular seam stays open (level L is missing on
+// [nz-1-L, nz) and [0, L+1)) until the last band has arrived; it is closed level by level at the end.  For long jobs
+// only the first and the last SKEW levels are skewed (enough kernel time per band to hide the copies) and the levels
+// in between run as whole-lattice launches.  Every launch is the same kernel restricted to a z range (Geom::zc), so the
+// result is bit-identical to the serial form.
 namespace {
-struct Pipeline {
+template <typename real>
+struct SkewJob {
     rflbm* h;
-    int C, CH, K;
-    int* level;                   // -1: not initialised, L >= 0: L steps done
-    cudaEvent_t* up;              // chunk uploaded
     const void *d_rho, *d_u;      // device fields for init (NULL: uniform start)
     int rc;
-    int za(int c) const { return c * CH; }
-    int zn(int c) const { return (c == C - 1) ? h->nz - c * CH : CH; }
-    int prev(int c) const { return (c + C - 1) % C; }
-    int next(int c) const { return (c + 1) % C; }
-    void range(int c) { h->zc = za(c); h->zn = zn(c); }
-    template <typename real> void init(int c)
+    // bring layers [a, b) from level L-1 to level L (L = 0: initialise from the uploaded fields)
+    void level(int L, int a, int b)
     {
-        if (rc != RFLBM_OK) return;
-        range(c);
-        rc = do_init<real>(h, d_rho, d_u);
-        level[c] = 0;
-    }
-    template <typename real> void step(int c)
-    {
-        if (rc != RFLBM_OK) return;
-        range(c);
-        h->t = (uint64_t)level[c];
-        h->cur = level[c] & 1;
-        rc = launch_step_once<real>(h);
-        level[c] += 1;
-    }
-    bool can_step(int c) const
-    {
-        return level[c] >= 0 && level[c] < K && level[prev(c)] >= level[c] && level[next(c)] >= level[c];
-    }
-    // everything that is possible right now, lowest levels first (the pyramid behind the upload front)
-    template <typename real> void greedy()
-    {
-        for (bool progressed = true; progressed && rc == RFLBM_OK;) {
-            progressed = false;
-            for (int c = 0; c < C; ++c)
-                if (can_step(c)) { step<real>(c); progressed = true; }
+        if (rc != RFLBM_OK || b <= a) return;
+        h->zc = a; h->zn = b - a;
+        if (L == 0) {
+            rc = do_init<real>(h, d_rho, d_u);
+        } else {
+            h->t = (uint64_t)(L - 1);
+            h->cur = (L - 1) & 1;
+            rc = launch_step_once<real>(h);
         }
     }
-    // bring chunk c to level L (all chunks are initialised): its neighbours first, one level below
-    template <typename real> void advance_to(int c, int L)
+    // Levels base+1 .. base+n over the ring of nz layers, in bands of CH layers.  ready(U) is called before anything
+    // that needs layers [0, U) of level `base` (the upload pass waits for the copy there; for a level that is complete
+    // everywhere it does nothing); emit(a, b) is called once for every range of layers whose level base+n is final on
+    // [a-1, b+1) (the moments can be taken).
+    template <typename Ready, typename Emit>
+    void pass(int base, int n, int CH, Ready ready, Emit emit)
     {
-        while (level[c] < L && rc == RFLBM_OK) {
-            advance_to<real>(prev(c), level[c]);
-            advance_to<real>(next(c), level[c]);
-            step<real>(c);
+        const int nz = h->nz;
+        int* hi = new (std::nothrow) int[n + 1];             // level base+i is done on [i, hi[i])
+        if (!hi) { rc = RFLBM_ENOMEM; return; }
+        for (int i = 0; i <= n; ++i) hi[i] = i;
+        int out_hi = n + 1;                                  // emitted so far: [n+1, out_hi)
+        for (int U = (CH < nz ? CH : nz);; U = (U + CH < nz ? U + CH : nz)) {
+            ready(U);
+            for (int i = 1; i <= n && i < U - i; ++i)
+                if (U - i > hi[i]) { level(base + i, hi[i], U - i); hi[i] = U - i; }
+            if (hi[n] - 1 > out_hi) { emit(out_hi, hi[n] - 1); out_hi = hi[n] - 1; }
+            if (U == nz) break;
         }
+        for (int i = 1; i <= n; ++i) {                       // the seam, level by level
+            if (hi[i] <= i) level(base + i, 0, nz);
+            else { level(base + i, hi[i], nz); level(base + i, 0, i); }
+        }
+        if (out_hi <= n + 1) emit(0, nz);
+        else { emit(out_hi, nz); emit(0, n + 1); }
+        delete[] hi;
     }
 };
 }  // namespace
@@ -631,80 +630,83 @@ static int run_host_pipelined(rflbm* h, const void* rho_host, const void* u_host
                               void* u_out_host, char* d_rho, char* d_u, size_t fb)
 {
     const size_t es = sizeof(real);
-    // 32 chunks: measured at 512^3, K = 20 (e2e ms): 16 chunks 308, 24: 284, 32: 271, 64: 293 — finer chunks make
-    // a taller pyramid of steps behind the upload front, but smaller launches fill the 148 SMs worse
+    // bands: at most 32, and thick enough that one band launch is ~8 waves of blocks (148 SMs x 3 blocks of the fp64 kernel;
+    // 8 rows per block in a band launch), at least 4 bands where the lattice has the layers: 16 layers at 512^3 (measured
+    // there, K = 20: 8 / 12 / 16 / 32 / 48 bands 240 / 239 / 237 / 238 / 243 ms), 56 at 256^3
     constexpr int MAXC = 32;
-    const int CH = (h->nz + MAXC - 1) / MAXC, C = (h->nz + CH - 1) / CH;
+    // levels skewed at either end of a long job: a band of CH layers costs SKEW launches of ~1/32 step each, which has to
+    // cover the copy of the band (2.4 ms of PCIe time against 0.3 ms per band and level at 512^3 fp64)
+    constexpr int SKEW = 12;
+    const int K = nsteps;
+    const int tx = h->tma_tx ? h->tma_tx : 128;
+    const long long blocks_per_layer = (long long)((h->nx + tx - 1) / tx) * ((h->ny + 7) / 8);
+    int CH = (h->nz + MAXC - 1) / MAXC;
+    const int thick = (int)std::min<long long>((8 * 444 + blocks_per_layer - 1) / blocks_per_layer, h->nz);
+    if (thick > CH) CH = thick;
+    if (CH > h->nz / 4) CH = h->nz / 4 > 0 ? h->nz / 4 : 1;
+    const int C = (h->nz + CH - 1) / CH;
     const size_t layer = (size_t)h->nx * h->ny * es;
-    int level[MAXC];
-    cudaEvent_t up[MAXC], mom[MAXC];
-    for (int c = 0; c < C; ++c) {
-        level[c] = -1;
-        cudaEventCreateWithFlags(&up[c], cudaEventDisableTiming);
-        cudaEventCreateWithFlags(&mom[c], cudaEventDisableTiming);
-    }
-    Pipeline p{h, C, CH, nsteps, level, up, rho_host ? d_rho : nullptr, rho_host ? d_u : nullptr, RFLBM_OK};
-    // a chunk launch is 1/32 of the lattice: finer blocks (8 rows instead of 16) keep its last wave of blocks short
+    cudaEvent_t up[MAXC], start, mom;
+    for (int c = 0; c < C; ++c) cudaEventCreateWithFlags(&up[c], cudaEventDisableTiming);
+    cudaEventCreateWithFlags(&start, cudaEventDisableTiming);
+    cudaEventCreateWithFlags(&mom, cudaEventDisableTiming);
+    SkewJob<real> job{h, rho_host ? d_rho : nullptr, rho_host ? d_u : nullptr, RFLBM_OK};
+    // a band launch is small: finer blocks (8 rows instead of 16) keep its last wave of blocks short
     const int rows_full = h->tma_rows;
-    h->tma_rows = 8;
     cudaStream_t cs = h->copy_stream;
     int rc = RFLBM_OK;
     // the copy stream starts after whatever the caller has already enqueued on the handle's stream
-    cudaEvent_t start;
-    cudaEventCreateWithFlags(&start, cudaEventDisableTiming);
     cudaEventRecord(start, h->stream);
     cudaStreamWaitEvent(cs, start, 0);
     // ---- uploads, in z order
     for (int c = 0; c < C && rc == RFLBM_OK; ++c) {
         if (rho_host) {
-            const size_t off = (size_t)p.za(c) * layer, len = (size_t)p.zn(c) * layer;
+            const size_t off = (size_t)c * CH * layer, len = (size_t)((c == C - 1 ? h->nz - c * CH : CH)) * layer;
             rc = check_cuda(h, cudaMemcpyAsync(d_rho + off, (const char*)rho_host + off, len, cudaMemcpyHostToDevice, cs), "H2D rho");
             for (int k = 0; k < 3 && rc == RFLBM_OK; ++k)
                 rc = check_cuda(h, cudaMemcpyAsync(d_u + k * fb + off, (const char*)u_host + k * fb + off, len, cudaMemcpyHostToDevice, cs), "H2D u");
         }
         cudaEventRecord(up[c], cs);
     }
-    // ---- init behind the upload front, steps behind the init front
-    for (int a = 2; a < C && rc == RFLBM_OK; ++a) {
-        cudaStreamWaitEvent(h->stream, up[a], 0);          // chunks a-2, a-1, a are on the device
-        p.template init<real>(a - 1);
-        p.template greedy<real>();
-    }
-    p.template init<real>(C - 1);                           // needs chunk 0: the periodic wrap closes the ring last
-    p.template init<real>(0);
-    // ---- finish chunk after chunk; moments and download of a finished chunk overlap the stepping of the others
-    int next_out = 0;
-    auto flush_outputs = [&](int upto) {                   // chunks < upto whose neighbours are finished too
-        for (; next_out < upto && p.rc == RFLBM_OK; ++next_out) {
-            const int c = next_out;
-            p.range(c);
-            h->t = (uint64_t)nsteps; h->cur = nsteps & 1;
-            p.rc = do_moments<real>(h, d_rho, d_u);
-            cudaEventRecord(mom[c], h->stream);
-            cudaStreamWaitEvent(cs, mom[c], 0);
-            const size_t off = (size_t)p.za(c) * layer, len = (size_t)p.zn(c) * layer;
-            cudaMemcpyAsync((char*)rho_out_host + off, d_rho + off, len, cudaMemcpyDeviceToHost, cs);
-            for (int k = 0; k < 3; ++k)
-                cudaMemcpyAsync((char*)u_out_host + k * fb + off, d_u + k * fb + off, len, cudaMemcpyDeviceToHost, cs);
-        }
+    auto uploaded = [&](int U) { cudaStreamWaitEvent(h->stream, up[(U + CH - 1) / CH - 1], 0); };
+    auto nothing = [](int) {};
+    auto keep = [](int, int) {};
+    // moments of layers [a, b) at the final level, then their way back to the host behind an event
+    auto output = [&](int a, int b) {
+        if (job.rc != RFLBM_OK || b <= a) return;
+        h->zc = a; h->zn = b - a;
+        h->t = (uint64_t)K; h->cur = K & 1;
+        job.rc = do_moments<real>(h, d_rho, d_u);
+        cudaEventRecord(mom, h->stream);
+        cudaStreamWaitEvent(cs, mom, 0);
+        const size_t off = (size_t)a * layer, len = (size_t)(b - a) * layer;
+        cudaMemcpyAsync((char*)rho_out_host + off, d_rho + off, len, cudaMemcpyDeviceToHost, cs);
+        for (int k = 0; k < 3; ++k)
+            cudaMemcpyAsync((char*)u_out_host + k * fb + off, d_u + k * fb + off, len, cudaMemcpyDeviceToHost, cs);
     };
-    for (int c = 0; c < C && p.rc == RFLBM_OK; ++c) {
-        p.template advance_to<real>(c, nsteps);
-        if (c >= 1 && c + 1 < C) {                          // chunk c-1 can go out once c-2, c-1, c are finished
-            if (c == 1) p.template advance_to<real>(C - 1, nsteps);   // chunk 0 also needs its other neighbour
-            flush_outputs(c);
+    if (C > MAXC) rc = fail(h, RFLBM_EINVAL, "rflbm_run_host: %d bands", C);       // cannot happen: CH >= nz / 32
+    if (rc == RFLBM_OK) {
+        h->tma_rows = 8;
+        if (K <= 2 * SKEW) {
+            job.pass(-1, K + 1, CH, uploaded, output);              // one pass: init and all K steps behind the upload front
+        } else {
+            job.pass(-1, SKEW + 1, CH, uploaded, keep);             // init and the first SKEW steps behind the upload front
+            h->tma_rows = rows_full;
+            for (int L = SKEW + 1; L <= K - SKEW; ++L) job.level(L, 0, h->nz);      // whole-lattice launches
+            h->tma_rows = 8;
+            job.pass(K - SKEW, SKEW, CH, nothing, output);          // the last SKEW steps with the download behind them
         }
     }
-    flush_outputs(C);
-    rc = (rc != RFLBM_OK) ? rc : p.rc;
+    rc = (rc != RFLBM_OK) ? rc : job.rc;
     // ---- state of the handle: as after rflbm_init + rflbm_step(nsteps)
     h->zc = 0; h->zn = h->nz;
     h->tma_rows = rows_full;
     h->t = (uint64_t)nsteps; h->cur = nsteps & 1; h->aa_phase = 0; h->inited = true;
     after_state_change(h);
     cudaError_t e1 = cudaStreamSynchronize(cs), e2 = cudaStreamSynchronize(h->stream);
-    for (int c = 0; c < C; ++c) { cudaEventDestroy(up[c]); cudaEventDestroy(mom[c]); }
+    for (int c = 0; c < C; ++c) cudaEventDestroy(up[c]);
     cudaEventDestroy(start);
+    cudaEventDestroy(mom);
     if (rc != RFLBM_OK) return rc;
     rc = check_cuda(h, e1, "cudaStreamSynchronize (copy stream)");
     return rc != RFLBM_OK ? rc : check_cuda(h, e2, "cudaStreamSynchronize");

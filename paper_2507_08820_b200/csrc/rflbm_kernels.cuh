@@ -274,7 +274,7 @@ __device__ __forceinline__ long long input_index(const Geom& G, int ghost_in, in
 }
 
 // P[q](s) = S[q](s + c_q), or S[26-q](s) when s + c_q is solid; solid nodes store S[q](s) unchanged.
-// `in` is canonical; written to both A and B buffers so that the never-updated solid layers agree.
+// `in` is canonical; the never-updated solid layers are written to both A and B buffers so that they agree.
 // AA scheme (P.aa): the natural layout P[q](s) = S[q](s), one buffer (bufB == nullptr).
 template <typename real, bool WALLS>
 __global__ void __launch_bounds__(128)
@@ -302,7 +302,8 @@ import_kernel(const real* __restrict__ in, real* __restrict__ bufA, real* __rest
         }
         const real v = in[from];
         bufA[(long long)q * G.QS + i.s] = v;
-        if (bufB != nullptr) bufB[(long long)q * G.QS + i.s] = v;
+        // the second A-B buffer only needs the solid layers (never updated, R12): the first step overwrites every fluid site
+        if (WALLS && solid && bufB != nullptr) bufB[(long long)q * G.QS + i.s] = v;
     }
 }
 
@@ -346,7 +347,8 @@ init_kernel(const real* __restrict__ rho, const real* __restrict__ u, double rho
         }
         const real v = (real)__dmul_rn(__dmul_rn(__dmul_rn(r, phi1d(cx, ux)), phi1d(cy, uy)), phi1d(cz, uz));
         bufA[(long long)q * G.QS + i.s] = v;
-        if (bufB != nullptr) bufB[(long long)q * G.QS + i.s] = v;
+        // the second A-B buffer only needs the solid layers (never updated, R12): the first step overwrites every fluid site
+        if (WALLS && solid && bufB != nullptr) bufB[(long long)q * G.QS + i.s] = v;
     }
 }
 

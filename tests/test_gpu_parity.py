@@ -202,11 +202,16 @@ def test_run_host_matches_device_path():
 @pytest.mark.parametrize("shape,prec,walls,force,nsteps", [
     ((24, 10, 6), binding.F64, False, None, 20), ((40, 6, 70), binding.F64, True, (1e-5, 0.0, 2e-6), 9),
     ((130, 5, 33), binding.F32, False, None, 13), ((9, 4, 3), binding.F64, False, None, 5),
-    ((36, 4, 40), binding.F64, False, None, 0), ((36, 4, 40), binding.F64, True, None, 1)])
+    ((36, 4, 40), binding.F64, False, None, 0), ((36, 4, 40), binding.F64, True, None, 1),
+    ((40, 6, 70), binding.F64, True, (1e-5, 0.0, 2e-6), 30), ((36, 4, 40), binding.F64, False, None, 25),
+    ((9, 4, 5), binding.F64, False, None, 40), ((130, 5, 200), binding.F32, False, None, 26),
+    ((33, 4, 64), binding.F64, False, None, 24), ((32, 3, 129), binding.F64, True, None, 31)])
 def test_run_host_pipelined_is_bit_identical_to_serial(shape, prec, walls, force, nsteps):
-    """rflbm_run_host with a copy stream (z-chunked upload / init / steps behind the upload front / chunked download)
-    against the serial form of the same call: bit-identical moments AND bit-identical final state of the handle;
-    chunk sizes 1..3 layers with a ragged last chunk, walls, force, fp32, 0 and 1 steps."""
+    """rflbm_run_host with a copy stream (time-skewed along z: every band of uploaded layers advances every level, the
+    ring's seam is closed at the end, moments leave behind the last level; more than 24 steps: skewed ends around
+    whole-lattice launches) against the serial form of the same call: bit-identical moments AND bit-identical final
+    state of the handle; bands of 1..7 layers with a ragged last band, walls, force, fp32, 0 and 1 steps, more steps
+    than layers."""
     torch = torch_()
     nx, ny, nz = shape
     dt = torch.float64 if prec == binding.F64 else torch.float32
