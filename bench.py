@@ -56,6 +56,9 @@ def parse_args():
                         "height with the faces exchanged every step (paper_2507_08820_b200/slab.py; PAPER.md:292, :300)")
     p.add_argument("--no-e2e", action="store_true")
     p.add_argument("--no-sustained", action="store_true")
+    p.add_argument("--aux", action="store_true",
+                   help="time the other device calls of the boundary (init, moments, stress, diagnostics, get/set_populations) "
+                        "at the bench size instead of the step; one JSON line")
     p.add_argument("--e2e-serial", action="store_true")
     p.add_argument("--no-cpu", action="store_true")
     p.add_argument("--cpu-seconds", type=float, default=12.0)
@@ -379,10 +382,55 @@ def run_ours(args):
     return 0
 
 
+def run_aux(args):
+    """The calls of include/rflbm.h around the step: device time and algorithmic bytes of each at
+    the bench size, thermalised state, best of 5 (CUDA events on the handle's stream)."""
+    import torch
+    from paper_2507_08820_b200 import binding
+    dev = torch.device("cuda:0")
+    n = args.size
+    nx, ny, nz = (int(v) for v in args.shape.split(",")) if args.shape else (n, n, n)
+    prec = binding.F64 if args.precision == "f64" else binding.F32
+    es = 8 if prec == binding.F64 else 4
+    N = nx * ny * nz
+    sim = binding.Rflbm(nx, ny, nz, WORKLOAD["tau"], args.kT, WORKLOAD["rho0"], WORKLOAD["seed"], prec, device=dev,
+                        scheme=binding.SCHEME_AA if args.scheme == "aa" else binding.SCHEME_AB)
+    sim.init()
+    sim.step(5)
+    dt = sim.dtype
+    rho = torch.empty((nz, ny, nx), dtype=dt, device=dev); u = torch.empty((3, nz, ny, nx), dtype=dt, device=dev)
+    pi = torch.empty((6, nz, ny, nx), dtype=dt, device=dev)
+    f = torch.empty((27, nz, ny, nx), dtype=dt, device=dev)
+    sim.get_populations(f)
+    # (call, values read per site, values written per site)
+    calls = [("rflbm_moments", lambda: sim.moments(rho, u), 27, 4), ("rflbm_stress", lambda: sim.stress(pi), 27, 6),
+             ("rflbm_diagnostics", lambda: sim.diagnostics(), 27, 0), ("rflbm_get_populations", lambda: sim.get_populations(f), 27, 27),
+             ("rflbm_set_populations", lambda: sim.set_populations(f, 5), 27, 27),
+             ("rflbm_init(rho,u)", lambda: sim.init(rho, u), 4, 27), ("rflbm_init(NULL)", lambda: sim.init(), 0, 27)]
+    peak, peak_src = hbm_peak()
+    out = {}
+    for name, fn, nr, nw in calls:
+        best = None
+        for _ in range(5):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize(dev)
+            e0.record(sim.stream); fn(); e1.record(sim.stream)
+            torch.cuda.synchronize(dev)
+            ms = e0.elapsed_time(e1)
+            best = ms if best is None else min(best, ms)
+        gbs = (nr + nw) * es * N / (best * 1e-3) / 1e9
+        out[name] = {"ms": best, "bytes_per_site": (nr + nw) * es, "gbs": gbs, "frac": gbs / peak}
+    print(json.dumps({"aux": out, "config": {"workload": f"{nx}x{ny}x{nz} {args.precision} {args.scheme}"}, "peak_gbs": peak,
+                      "peak_source": peak_src, "note": "rflbm_diagnostics includes its host read-back of ten sums"}))
+    return 0
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.aux:
+        return run_aux(args)
     return run_ours(args)
 
 
