@@ -1,0 +1,79 @@
+"""Table III of the paper at ITS OWN settings on one B200 (not collected by pytest: 10 minutes of GPU time per row).
+
+    python tests/table_III_full_scale.py --model reg --tau 0.5001,0.51,1.0,50.0
+    python tests/table_III_full_scale.py --model bgk --tau 0.505,10.0,50.0
+
+PAPER.md:252-260: 256^3 periodic lattice, fp64, kT = 1/3000, uniform rho = 1 start, 5e5 steps, rho, rho u and Pi_ab saved
+every 5 000 steps (100 snapshots); ER = variance of the field over the lattice / (rho0 kT b_k / c_s^2), averaged over the
+snapshots.  The fields come from rflbm_moments and rflbm_stress; the variances are torch reductions on the device.
+Prints every row beside the printed one (tests/golden/table_III_regflbm.txt, table_III_bgkflbm.txt) and exits non-zero
+if a Reg-FLBM row is further than 0.01 (0.04 for tau < 0.505) from the paper's; the BGK column is reported only
+(reading R19).  Results of this build: profiles/r02_table_III_full.md."""
+import argparse
+import os
+import sys
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+sys.path.insert(0, ROOT)
+
+
+def full_scale_er(tau, model, n=256, kT=1.0 / 3000.0, nsnap=100, every=5000):
+    """ER(rho, j, Pi_aa, Pi_ab) by the paper's protocol"""
+    import torch
+    from paper_2507_08820_b200 import binding
+    sim = binding.Rflbm(n, n, n, tau, kT, 1.0, 2507)
+    sim.set_model(model)
+    sim.init()
+    rho = torch.empty((n, n, n), dtype=torch.float64, device="cuda")
+    u = torch.empty((3, n, n, n), dtype=torch.float64, device="cuda")
+    pi = torch.empty((6, n, n, n), dtype=torch.float64, device="cuda")        # xx, yy, zz, xy, xz, yz
+    er = []
+    for _ in range(nsnap):
+        sim.step(every)
+        sim.moments(rho, u)
+        sim.stress(pi)
+        j = u * rho
+        er.append([float(rho.var(unbiased=False)) / (3 * kT),
+                   float(j.reshape(3, -1).var(dim=1, unbiased=False).mean()) / kT,
+                   float(pi[:3].reshape(3, -1).var(dim=1, unbiased=False).mean()) / (2.0 / 3.0 * kT),
+                   float(pi[3:].reshape(3, -1).var(dim=1, unbiased=False).mean()) / (1.0 / 3.0 * kT)])
+    assert sim.step_count == nsnap * every
+    sim.close()
+    return np.mean(er, axis=0)
+
+
+def main():
+    from paper_2507_08820_b200 import binding
+    p = argparse.ArgumentParser()
+    p.add_argument("--model", default="reg", choices=["reg", "bgk"])
+    p.add_argument("--tau", required=True, help="comma-separated relaxation times (rows of Table III)")
+    p.add_argument("--size", type=int, default=256)
+    p.add_argument("--snapshots", type=int, default=100)
+    p.add_argument("--every", type=int, default=5000)
+    a = p.parse_args()
+    golden = os.path.join(ROOT, "tests", "golden", "table_III_regflbm.txt" if a.model == "reg" else "table_III_bgkflbm.txt")
+    printed = {float(ln.split()[0]): [float(v) for v in ln.split()[1:]] for ln in open(golden)
+               if ln.strip() and not ln.startswith("#")}
+    model = binding.MODEL_REG if a.model == "reg" else binding.MODEL_BGK
+    print(f"   tau    {a.model} ER(rho, j, Pi_aa, Pi_ab) here ({a.size}^3, {a.snapshots * a.every} steps, {a.snapshots} snapshots)"
+          "   |  Table III", flush=True)
+    bad = []
+    for tau in [float(v) for v in a.tau.split(",")]:
+        er = full_scale_er(tau, model, a.size, 1.0 / 3000.0, a.snapshots, a.every)
+        paper = printed[tau]
+        print(f"{tau:8.4f}  " + "  ".join(f"{v:6.4f}" for v in er) + "   |  " + "  ".join(f"{v:5.3f}" for v in paper), flush=True)
+        ok = bool(np.isfinite(er).all())
+        if a.model == "reg":
+            ok = ok and float(np.abs(er - np.array(paper)).max()) < (0.04 if tau < 0.505 else 0.01)
+        if not ok:
+            bad.append(tau)
+    if bad:
+        print("rows outside the bracket:", bad)
+        return 1
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())
