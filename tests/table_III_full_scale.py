@@ -19,26 +19,27 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 sys.path.insert(0, ROOT)
 
 
-def full_scale_er(tau, model, n=256, kT=1.0 / 3000.0, nsnap=100, every=5000):
+def full_scale_er(tau, model, n=256, kT=1.0 / 3000.0, nsnap=100, every=5000, precision=None):
     """ER(rho, j, Pi_aa, Pi_ab) by the paper's protocol"""
     import torch
     from paper_2507_08820_b200 import binding
-    sim = binding.Rflbm(n, n, n, tau, kT, 1.0, 2507)
+    sim = binding.Rflbm(n, n, n, tau, kT, 1.0, 2507, binding.F64 if precision is None else precision)
     sim.set_model(model)
     sim.init()
-    rho = torch.empty((n, n, n), dtype=torch.float64, device="cuda")
-    u = torch.empty((3, n, n, n), dtype=torch.float64, device="cuda")
-    pi = torch.empty((6, n, n, n), dtype=torch.float64, device="cuda")        # xx, yy, zz, xy, xz, yz
+    rho = torch.empty((n, n, n), dtype=sim.dtype, device="cuda")
+    u = torch.empty((3, n, n, n), dtype=sim.dtype, device="cuda")
+    pi = torch.empty((6, n, n, n), dtype=sim.dtype, device="cuda")            # xx, yy, zz, xy, xz, yz
     er = []
     for _ in range(nsnap):
         sim.step(every)
         sim.moments(rho, u)
         sim.stress(pi)
-        j = u * rho
-        er.append([float(rho.var(unbiased=False)) / (3 * kT),
+        r64, p64 = rho.double(), pi.double()                                  # fp32 storage (R14): statistics in fp64
+        j = u.double() * r64
+        er.append([float(r64.var(unbiased=False)) / (3 * kT),
                    float(j.reshape(3, -1).var(dim=1, unbiased=False).mean()) / kT,
-                   float(pi[:3].reshape(3, -1).var(dim=1, unbiased=False).mean()) / (2.0 / 3.0 * kT),
-                   float(pi[3:].reshape(3, -1).var(dim=1, unbiased=False).mean()) / (1.0 / 3.0 * kT)])
+                   float(p64[:3].reshape(3, -1).var(dim=1, unbiased=False).mean()) / (2.0 / 3.0 * kT),
+                   float(p64[3:].reshape(3, -1).var(dim=1, unbiased=False).mean()) / (1.0 / 3.0 * kT)])
     assert sim.step_count == nsnap * every
     sim.close()
     return np.mean(er, axis=0)
@@ -49,6 +50,7 @@ def main():
     p = argparse.ArgumentParser()
     p.add_argument("--model", default="reg", choices=["reg", "bgk"])
     p.add_argument("--tau", required=True, help="comma-separated relaxation times (rows of Table III)")
+    p.add_argument("--precision", default="f64", choices=["f64", "f32"], help="f32: fp32 storage and arithmetic (R14)")
     p.add_argument("--size", type=int, default=256)
     p.add_argument("--snapshots", type=int, default=100)
     p.add_argument("--every", type=int, default=5000)
@@ -57,11 +59,12 @@ def main():
     printed = {float(ln.split()[0]): [float(v) for v in ln.split()[1:]] for ln in open(golden)
                if ln.strip() and not ln.startswith("#")}
     model = binding.MODEL_REG if a.model == "reg" else binding.MODEL_BGK
-    print(f"   tau    {a.model} ER(rho, j, Pi_aa, Pi_ab) here ({a.size}^3, {a.snapshots * a.every} steps, {a.snapshots} snapshots)"
+    print(f"   tau    {a.model} {a.precision} ER(rho, j, Pi_aa, Pi_ab) here ({a.size}^3, {a.snapshots * a.every} steps, {a.snapshots} snapshots)"
           "   |  Table III", flush=True)
     bad = []
     for tau in [float(v) for v in a.tau.split(",")]:
-        er = full_scale_er(tau, model, a.size, 1.0 / 3000.0, a.snapshots, a.every)
+        er = full_scale_er(tau, model, a.size, 1.0 / 3000.0, a.snapshots, a.every,
+                           binding.F64 if a.precision == "f64" else binding.F32)
         paper = printed[tau]
         print(f"{tau:8.4f}  " + "  ".join(f"{v:6.4f}" for v in er) + "   |  " + "  ".join(f"{v:5.3f}" for v in paper), flush=True)
         ok = bool(np.isfinite(er).all())
