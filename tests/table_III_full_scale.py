@@ -19,7 +19,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 sys.path.insert(0, ROOT)
 
 
-def full_scale_er(tau, model, n=256, kT=1.0 / 3000.0, nsnap=100, every=5000, precision=None):
+def full_scale_er(tau, model, n=256, kT=1.0 / 3000.0, nsnap=100, every=5000, precision=None, trace=False):
     """ER(rho, j, Pi_aa, Pi_ab) by the paper's protocol"""
     import torch
     from paper_2507_08820_b200 import binding
@@ -42,6 +42,10 @@ def full_scale_er(tau, model, n=256, kT=1.0 / 3000.0, nsnap=100, every=5000, pre
                    float(p64[3:].reshape(3, -1).var(dim=1, unbiased=False).mean()) / (1.0 / 3.0 * kT)])
     assert sim.step_count == nsnap * every
     sim.close()
+    if trace:                                                                 # is the run stationary? means over tenths of the run
+        for k in range(0, nsnap, max(1, nsnap // 10)):
+            part = np.mean(er[k:k + max(1, nsnap // 10)], axis=0)
+            print(f"      snapshots {k + 1:3d}-{min(nsnap, k + max(1, nsnap // 10)):3d}: " + "  ".join(f"{v:6.4f}" for v in part), flush=True)
     return np.mean(er, axis=0)
 
 
@@ -51,6 +55,7 @@ def main():
     p.add_argument("--model", default="reg", choices=["reg", "bgk"])
     p.add_argument("--tau", required=True, help="comma-separated relaxation times (rows of Table III)")
     p.add_argument("--precision", default="f64", choices=["f64", "f32"], help="f32: fp32 storage and arithmetic (R14)")
+    p.add_argument("--trace", action="store_true", help="also print the means over every tenth of the snapshots")
     p.add_argument("--size", type=int, default=256)
     p.add_argument("--snapshots", type=int, default=100)
     p.add_argument("--every", type=int, default=5000)
@@ -64,7 +69,7 @@ def main():
     bad = []
     for tau in [float(v) for v in a.tau.split(",")]:
         er = full_scale_er(tau, model, a.size, 1.0 / 3000.0, a.snapshots, a.every,
-                           binding.F64 if a.precision == "f64" else binding.F32)
+                           binding.F64 if a.precision == "f64" else binding.F32, a.trace)
         paper = printed[tau]
         print(f"{tau:8.4f}  " + "  ".join(f"{v:6.4f}" for v in er) + "   |  " + "  ".join(f"{v:5.3f}" for v in paper), flush=True)
         ok = bool(np.isfinite(er).all())
