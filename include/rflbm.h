@@ -193,6 +193,38 @@ uint64_t rflbm_launch_count(const rflbm_t* h);
  * first step): a static string, what bench.py reports as roofline.kernel. */
 const char* rflbm_last_kernel(const rflbm_t* h);
 
+/* The sums of rflbm_diagnostics for a caller that CANNOT ALLOCATE device memory: no handle, no workspace, nothing
+ * allocated by the call (no cudaMalloc / cudaFree / allocating library routine, on the device or pinned).
+ * rflbm_diagnostics itself needs a handle whose workspace holds one or two complete population buffers (29-58 GB at
+ * 512^3 fp64).  A checkpoint inspector, an in-situ monitor or a plug-in that is handed a population field inside a
+ * process whose device memory is already spoken for (the simulation owns the HBM, the host application owns the pool),
+ * or that runs where cudaMalloc's device-wide synchronisation is not acceptable, has nowhere to get that from.  For
+ * such callers the reduction scratch is part of the library image: a file-scope __device__ array of 2.5 MiB
+ * (32 768 rows of 10 doubles + 1) that every GPU which loads librflbm.so carries until the process exits.
+ *   f_dev      in   canonical PRE-collision populations f[27][N] (device, `real` by `precision`; what
+ *                   rflbm_get_populations writes), N = nx*ny*nz, x fastest.  Borrowed for the duration of the call.
+ *   walls_z    in   non-zero: layers z = 0 and z = nz-1 are solid and excluded (R12); needs nz >= 3
+ *   g_host     in   acceleration g[3] (host) or NULL for none: the reported velocity is u = j/rho + g/2 (R13)
+ *   stream     in   cudaStream_t (as void*) on the CURRENT device; f_dev must live on the current device
+ *   out_host   out  { sum rho, sum rho u_x,y,z, mean u_x,y,z, var u_x,y,z } over the fluid sites, as rflbm_diagnostics
+ *   err_host   out  optional (may be NULL): err_len bytes that receive a NUL-terminated message on failure
+ * Limit: N <= rflbm_static_max_sites() = RFLBM_STATIC_MAX_SITES = 2^27 (512^3, the headline lattice).  Anything larger
+ * is refused with RFLBM_EINVAL and a message naming the limit, before any GPU work.  Other EINVAL: NULL f_dev /
+ * out_host, sizes < 1, unknown precision, non-finite g, f_dev not device memory of the current device.  ECUDA: a CUDA
+ * call failed.
+ * The call enqueues two kernels and an 80-byte copy on `stream` and waits for the stream (host-synchronous, like
+ * rflbm_diagnostics).  No atomics: repeated calls on the same field return the same bits.
+ * First call on a device: looks up the device address of the static array (cudaGetSymbolAddress, cached per device);
+ * with the runtime's lazy module loading this is also the moment the array and the two kernels take their device
+ * memory.  Make that first call outside any stream capture.
+ * Sharing: all calls on one GPU, from any thread or handle, use the same array, and it keeps what the last call left in
+ * it.  Nothing in it needs to start at zero (every row a call reads it has written itself first), but two calls that
+ * overlap on the GPU (different streams, different threads) race on it and return garbage: serialise them. */
+#define RFLBM_STATIC_MAX_SITES 134217728LL
+long long rflbm_static_max_sites(void);
+int rflbm_diagnostics_static(const void* f_dev, int nx, int ny, int nz, int precision, int walls_z, const double* g_host,
+                             void* cuda_stream, double out_host[10], char* err_host, size_t err_len);
+
 uint64_t rflbm_step_count(const rflbm_t* h);
 const char* rflbm_last_error(const rflbm_t* h);
 

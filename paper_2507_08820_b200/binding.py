@@ -54,6 +54,9 @@ SYMBOLS = {
     "rflbm_step_count": (_u64, [_vp]),
     "rflbm_last_error": (C.c_char_p, [_vp]),
     "rflbm_destroy": (_i32, [_vp]),
+    "rflbm_static_max_sites": (C.c_longlong, []),
+    "rflbm_diagnostics_static": (_i32, [_vp, _i32, _i32, _i32, _i32, _i32, C.POINTER(_dbl), _vp, C.POINTER(_dbl),
+                                        C.c_char_p, _sz]),
 }
 
 
@@ -82,6 +85,31 @@ def load():
 
 def _ptr(t):
     return 0 if t is None else t.data_ptr()
+
+
+def diagnostics_static(f, walls=False, g=None, stream=None):
+    """rflbm_diagnostics_static: the ten numbers of Rflbm.diagnostics() for a canonical population tensor
+    f[27, nz, ny, nx] (CUDA, float64 or float32, contiguous) WITHOUT a handle or a workspace.
+
+    For code that may not allocate device memory (a checkpoint inspector or monitor inside a process whose HBM is
+    already taken, a plug-in that must stay out of the host's pool): the reduction scratch is a 2.5 MiB static array
+    inside librflbm.so, so neither this wrapper nor the library allocates anything on the device.  At most
+    rflbm_static_max_sites() = 2**27 sites; larger fields raise RflbmError(EINVAL).  Calls share the one array per GPU:
+    do not overlap them (include/rflbm.h)."""
+    import torch
+    lib = load()
+    assert f.is_cuda and f.is_contiguous() and f.dim() == 4 and f.shape[0] == Q, "f[27, nz, ny, nx] on the GPU"
+    assert f.dtype in (torch.float64, torch.float32)
+    nz, ny, nx = (int(v) for v in f.shape[1:])
+    out, err = (_dbl * 10)(), C.create_string_buffer(512)
+    gv = None if g is None else (_dbl * 3)(*(float(v) for v in g))
+    with torch.cuda.device(f.device):
+        st = stream if stream is not None else torch.cuda.current_stream(f.device)
+        rc = lib.rflbm_diagnostics_static(f.data_ptr(), nx, ny, nz, F64 if f.dtype == torch.float64 else F32, int(bool(walls)),
+                                          gv, st.cuda_stream, out, err, len(err))
+    if rc != OK:
+        raise RflbmError(rc, err.value.decode())
+    return list(out)
 
 
 class Rflbm:

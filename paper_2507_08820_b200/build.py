@@ -15,12 +15,12 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(CSRC, "librflbm.so")
-SOURCES = ["rflbm.cu", "rflbm_step_inst.cu"]
+SOURCES = ["rflbm.cu", "rflbm_step_inst.cu", "rflbm_static.cu"]
 HEADERS = ["rflbm_lattice.cuh", "rflbm_fastmath.cuh", "rflbm_rng.cuh", "rflbm_collide.cuh", "rflbm_kernels.cuh",
            "rflbm_step_tma.cuh", "rflbm_host.cuh", os.path.join("..", "..", "include", "rflbm.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC"]
 # (object name, source, extra defines)
-UNITS = [("rflbm.o", "rflbm.cu", [])] + [
+UNITS = [("rflbm.o", "rflbm.cu", []), ("rflbm_static.o", "rflbm_static.cu", [])] + [
     (f"step_{r}_{p}_{tx}.o", "rflbm_step_inst.cu", [f"-DRFLBM_INST_REAL={r}", f"-DRFLBM_INST_PHASE={p}", f"-DRFLBM_INST_TX={tx}"])
     for tx in (128, 0, 64, 32) for r in ("double", "float") for p in (0, 1, 2)]
 
