@@ -40,8 +40,10 @@ enum { RFLBM_OK = 0, RFLBM_EINVAL = -1, RFLBM_ESTATE = -2, RFLBM_ENOMEM = -3, RF
  * PAPER.md:52; ghost rate omega_g = 1, :215), thermal energy kT (Eq.9 :99; kT = 0 -> deterministic
  * Reg-LBM, :294), reference density rho0 (:252), Philox seed (R8) and precision.
  * Host only: no GPU work, no allocation on the device.
- * EINVAL: nx,ny,nz < 1, N >= 2^32, ny > 65535 * max(1, 128/nx rounded down to a power of two) or nz > 65535 (launch
- * grid limits), tau <= 0.5 or non-finite, kT < 0, rho0 <= 0, unknown precision, out NULL. */
+ * EINVAL: nx,ny,nz < 1, N >= 2^32, nx > RFLBM_MAX_NX (27 padded rows must fit a 32-bit row offset), ny > 65535 *
+ * max(1, 128/nx rounded down to a power of two) or nz > 65535 (launch grid limits), tau <= 0.5 or non-finite, kT < 0,
+ * rho0 <= 0, unknown precision, out NULL. */
+#define RFLBM_MAX_NX (2147483647 / 27 - 32) /* 79 536 399 */
 int rflbm_create(int nx, int ny, int nz, double tau, double kT, double rho0, uint64_t seed, int precision,
                  rflbm_t** out);
 
@@ -112,7 +114,8 @@ int rflbm_set_slab(rflbm_t* h, int z0, int nz_global);
  * (HIGH) post-collision populations of the boundary layer that the neighbour will pull (A-B, and AA after an even
  * step), or, after an odd AA step, the nine populations this slab pushed across the face, which the neighbour takes
  * home into its own boundary layer.  pack and unpack enqueue one small kernel on the handle's stream and return;
- * they are no-ops (RFLBM_OK) when nothing is pending.  ESTATE: not in slab mode, or before init. */
+ * they are no-ops (RFLBM_OK) when nothing is pending; a second rflbm_halo_unpack of a side that has
+ * already been unpacked since the last step is a no-op too (the face is consumed once).  ESTATE: not in slab mode, or before init. */
 enum { RFLBM_SIDE_LOW = 0, RFLBM_SIDE_HIGH = 1 };
 size_t rflbm_halo_bytes(const rflbm_t* h);
 int rflbm_halo_pending(const rflbm_t* h);
@@ -150,7 +153,7 @@ int rflbm_moments(rflbm_t* h, void* rho_dev, void* u_dev);
 int rflbm_stress(rflbm_t* h, void* pi_dev);
 
 /* Synchronises the stream.  out_host = { sum rho, sum rho u_x,y,z, mean u_x,y,z, var u_x,y,z } over fluid sites
- * (warp-shuffle + block reduction, fp64 accumulation). */
+ * (warp-shuffle + block reduction, fp64 accumulation).  A slab without a fluid site (one solid layer): all zeros. */
 int rflbm_diagnostics(rflbm_t* h, double out_host[10]);
 
 /* Canonical pre-collision populations f[27][N] (`real`, device) out of / into the handle.

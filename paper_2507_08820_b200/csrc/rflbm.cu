@@ -93,6 +93,8 @@ extern "C" int rflbm_create(int nx, int ny, int nz, double tau, double kT, doubl
     *out = nullptr;
     if (nx < 1 || ny < 1 || nz < 1) return RFLBM_EINVAL;
     if ((double)nx * (double)ny * (double)nz >= 4294967296.0) return RFLBM_EINVAL;
+    // Geom::px = 27 x the padded row length (nx rounded up by at most 31 elements) is an int in every kernel
+    if (nx > RFLBM_MAX_NX) return RFLBM_EINVAL;
     if (!std::isfinite(tau) || !(tau > 0.5)) return RFLBM_EINVAL;
     if (!std::isfinite(kT) || kT < 0.0) return RFLBM_EINVAL;
     if (!std::isfinite(rho0) || !(rho0 > 0.0)) return RFLBM_EINVAL;
@@ -502,8 +504,9 @@ extern "C" int rflbm_diagnostics(rflbm_t* h, double out_host[10])
     out_host[0] = s[0];
     for (int a = 0; a < 3; ++a) {
         out_host[1 + a] = s[1 + a];
-        out_host[4 + a] = s[4 + a] / nf;
-        out_host[7 + a] = s[7 + a] / nf - out_host[4 + a] * out_host[4 + a];
+        // a slab that owns nothing but a solid layer has no fluid site: sums 0, mean and variance reported as 0
+        out_host[4 + a] = nf > 0.0 ? s[4 + a] / nf : 0.0;
+        out_host[7 + a] = nf > 0.0 ? s[7 + a] / nf - out_host[4 + a] * out_host[4 + a] : 0.0;
     }
     return RFLBM_OK;
 }
@@ -818,6 +821,9 @@ static int do_halo(rflbm* h, int side, void* face_dev)
     if (!h->slab) return fail(h, RFLBM_ESTATE, "not in slab mode (rflbm_set_slab)");
     if (!h->inited) return fail(h, RFLBM_ESTATE, "halo call before init");
     if (h->halo_mode == HALO_NONE || (PACK && h->halo_done == 3)) return RFLBM_OK;    // nothing to exchange in this state
+    // a side that has already been unpacked since the last step is complete: unpacking again would, in HALO_HOME,
+    // overwrite nine populations of the boundary layer with whatever the face buffer holds by now
+    if (!PACK && (h->halo_done & ((side == RFLBM_SIDE_LOW) ? 1 : 2))) return RFLBM_OK;
     const HaloPlan p = halo_plan(h, side, PACK);
     if (!p.skip) {
         const Geom G = make_geom(h);

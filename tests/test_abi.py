@@ -98,6 +98,21 @@ def test_slab_and_grid_validation_host_side(lib):
     assert lib.rflbm_create(8, 70000, 1, 1.0, 0.0, 1.0, 0, binding.F64, C.byref(h)) == binding.OK
     lib.rflbm_destroy(h)
     assert lib.rflbm_create(1, 1, 70000, 1.0, 0.0, 1.0, 0, binding.F64, C.byref(h)) == binding.EINVAL
+    # row offsets are 32-bit: 27 x the padded row (nx rounded up by at most 31 elements) must fit an int, i.e.
+    # nx <= RFLBM_MAX_NX = INT_MAX/27 - 32.  80 000 000 x 2 x 1 has fewer than 2^32 sites and was accepted before.
+    max_nx = (2 ** 31 - 1) // 27 - 32
+    hdr = open(os.path.join(ROOT, "include", "rflbm.h")).read()
+    assert "#define RFLBM_MAX_NX (2147483647 / 27 - 32)" in hdr
+    assert lib.rflbm_create(80_000_000, 2, 1, 1.0, 0.0, 1.0, 0, binding.F64, C.byref(h)) == binding.EINVAL
+    assert lib.rflbm_create(max_nx + 1, 1, 1, 1.0, 0.0, 1.0, 0, binding.F32, C.byref(h)) == binding.EINVAL
+    for prec in (binding.F64, binding.F32):
+        assert lib.rflbm_create(max_nx, 2, 1, 1.0, 0.0, 1.0, 0, prec, C.byref(h)) == binding.OK
+        es = 8 if prec == binding.F64 else 4
+        line = 128 // es
+        px = (max_nx + line - 1) // line * line
+        assert 27 * px <= 2 ** 31 - 1                                                 # what Geom::px holds
+        assert lib.rflbm_workspace_bytes(h) == 2 * ((27 * px * 2 * es + 255) // 256 * 256) + 4096 + 12288
+        lib.rflbm_destroy(h)
 
 
 def test_no_environment_knobs_in_the_product():
