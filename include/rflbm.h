@@ -176,13 +176,21 @@ int rflbm_debug_rng(rflbm_t* h, uint64_t step, void* words_dev, void* normals_de
  * uploaded in up to 32 bands of consecutive layers; as soon as the layers [0, U) are on the device, the state after L steps
  * is completed on the layers [L+1, U-1-L) for EVERY L (a step reaches one layer up and down, so each level runs one layer
  * behind the level below it), and the moments of the layers that have reached step nsteps are downloaded while the rest
- * is still being uploaded or stepped; the triangular seam the periodic ring leaves open is closed at the end.  Jobs of
+ * is still being stepped (uploads and downloads share the copy stream and every upload is enqueued first, so the first
+ * download starts once the last band is up); the triangular seam the periodic ring leaves open is closed at the end.  Jobs of
  * more than 24 steps skew only the first and the last 12 steps and run the steps in between as whole-lattice launches.
  * Every launch is the same kernel restricted to a z range, so the results are bit-identical to the serial form.
  * Without a copy stream, in the AA scheme, or with nz < 3, everything runs one after the other on the handle's stream.
- * ESTATE in slab mode. */
+ * ESTATE in slab mode.  ECUDA: a copy, event or launch failed (text of the FIRST failure in rflbm_last_error); both
+ * streams are quiet when the call returns, and after a failed pipelined job the handle holds NO state (ESTATE until the
+ * next rflbm_init / rflbm_set_populations / rflbm_run_host) and the output buffers are unspecified. */
 int rflbm_run_host(rflbm_t* h, const void* rho_host, const void* u_host, int nsteps, void* rho_out_host,
                    void* u_out_host, void* scratch_dev, size_t scratch_bytes);
+
+/* Test hook: the nth_call-th checked CUDA call (event, copy, wait, synchronise; counted from 1) of the NEXT pipelined
+ * rflbm_run_host on this handle reports cudaErrorUnknown although it succeeded, so that the job's error path can be
+ * exercised without corrupting the device; 0 disarms.  The job clears it when it returns. */
+int rflbm_debug_inject_failure(rflbm_t* h, int nth_call);
 
 /* A second cudaStream_t (as void*), borrowed, on which rflbm_run_host issues its host<->device copies so that they
  * overlap the kernels on the handle's stream (the two are ordered by events the call creates and destroys).

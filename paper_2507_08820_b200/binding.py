@@ -49,6 +49,7 @@ SYMBOLS = {
     "rflbm_debug_rng": (_i32, [_vp, _u64, _vp, _vp]),
     "rflbm_run_host": (_i32, [_vp, _vp, _vp, _i32, _vp, _vp, _vp, _sz]),
     "rflbm_set_copy_stream": (_i32, [_vp, _vp]),
+    "rflbm_debug_inject_failure": (_i32, [_vp, _i32]),
     "rflbm_launch_count": (_u64, [_vp]),
     "rflbm_last_kernel": (C.c_char_p, [_vp]),
     "rflbm_step_count": (_u64, [_vp]),
@@ -254,6 +255,9 @@ class Rflbm:
             normals = t.empty((23,) + self.shape, dtype=self.dtype, device=self.device)
             self._ck(self.lib.rflbm_debug_rng(self.h, int(step), words.data_ptr(), normals.data_ptr()))
         return words, normals
+
+    def debug_inject_failure(self, nth_call):
+        self._ck(self.lib.rflbm_debug_inject_failure(self.h, int(nth_call)))
 
     def set_copy_stream(self, stream):
         """second torch stream for the copies of run_host (None: serial)"""

@@ -649,46 +649,57 @@ static int run_host_pipelined(rflbm* h, const void* rho_host, const void* u_host
     if (CH > h->nz / 4) CH = h->nz / 4 > 0 ? h->nz / 4 : 1;
     const int C = (h->nz + CH - 1) / CH;
     const size_t layer = (size_t)h->nx * h->ny * es;
-    cudaEvent_t up[MAXC], start, mom;
-    for (int c = 0; c < C; ++c) cudaEventCreateWithFlags(&up[c], cudaEventDisableTiming);
-    cudaEventCreateWithFlags(&start, cudaEventDisableTiming);
-    cudaEventCreateWithFlags(&mom, cudaEventDisableTiming);
+    // Every CUDA call below goes through ck(): the first failure is kept in job.rc (with its text in the handle), and
+    // everything after it is skipped (SkewJob::level and the lambdas test job.rc).
     SkewJob<real> job{h, rho_host ? d_rho : nullptr, rho_host ? d_u : nullptr, RFLBM_OK};
+    auto ck = [&](cudaError_t e, const char* what) {
+        if (h->inject_fail > 0 && --h->inject_fail == 0 && e == cudaSuccess) e = cudaErrorUnknown;    // rflbm_debug_inject_failure
+        if (e != cudaSuccess && job.rc == RFLBM_OK) job.rc = check_cuda(h, e, what);
+        return e == cudaSuccess;
+    };
+    cudaEvent_t up[MAXC], start = nullptr, mom = nullptr;
+    int n_up = 0;
+    if (C > MAXC) job.rc = fail(h, RFLBM_EINVAL, "rflbm_run_host: %d bands", C);       // cannot happen: CH >= nz / 32
+    while (job.rc == RFLBM_OK && n_up < C && ck(cudaEventCreateWithFlags(&up[n_up], cudaEventDisableTiming), "cudaEventCreate")) ++n_up;
+    if (job.rc == RFLBM_OK && !ck(cudaEventCreateWithFlags(&start, cudaEventDisableTiming), "cudaEventCreate")) start = nullptr;
+    if (job.rc == RFLBM_OK && !ck(cudaEventCreateWithFlags(&mom, cudaEventDisableTiming), "cudaEventCreate")) mom = nullptr;
     // a band launch is small: finer blocks (8 rows instead of 16) keep its last wave of blocks short
     const int rows_full = h->tma_rows;
     cudaStream_t cs = h->copy_stream;
-    int rc = RFLBM_OK;
     // the copy stream starts after whatever the caller has already enqueued on the handle's stream
-    cudaEventRecord(start, h->stream);
-    cudaStreamWaitEvent(cs, start, 0);
+    if (job.rc == RFLBM_OK) ck(cudaEventRecord(start, h->stream), "cudaEventRecord");
+    if (job.rc == RFLBM_OK) ck(cudaStreamWaitEvent(cs, start, 0), "cudaStreamWaitEvent (copy stream)");
     // ---- uploads, in z order
-    for (int c = 0; c < C && rc == RFLBM_OK; ++c) {
+    for (int c = 0; c < C && job.rc == RFLBM_OK; ++c) {
         if (rho_host) {
             const size_t off = (size_t)c * CH * layer, len = (size_t)((c == C - 1 ? h->nz - c * CH : CH)) * layer;
-            rc = check_cuda(h, cudaMemcpyAsync(d_rho + off, (const char*)rho_host + off, len, cudaMemcpyHostToDevice, cs), "H2D rho");
-            for (int k = 0; k < 3 && rc == RFLBM_OK; ++k)
-                rc = check_cuda(h, cudaMemcpyAsync(d_u + k * fb + off, (const char*)u_host + k * fb + off, len, cudaMemcpyHostToDevice, cs), "H2D u");
+            ck(cudaMemcpyAsync(d_rho + off, (const char*)rho_host + off, len, cudaMemcpyHostToDevice, cs), "H2D rho");
+            for (int k = 0; k < 3 && job.rc == RFLBM_OK; ++k)
+                ck(cudaMemcpyAsync(d_u + k * fb + off, (const char*)u_host + k * fb + off, len, cudaMemcpyHostToDevice, cs), "H2D u");
         }
-        cudaEventRecord(up[c], cs);
+        if (job.rc == RFLBM_OK) ck(cudaEventRecord(up[c], cs), "cudaEventRecord (upload)");
     }
-    auto uploaded = [&](int U) { cudaStreamWaitEvent(h->stream, up[(U + CH - 1) / CH - 1], 0); };
+    auto uploaded = [&](int U) {
+        if (job.rc == RFLBM_OK) ck(cudaStreamWaitEvent(h->stream, up[(U + CH - 1) / CH - 1], 0), "cudaStreamWaitEvent (upload)");
+    };
     auto nothing = [](int) {};
     auto keep = [](int, int) {};
-    // moments of layers [a, b) at the final level, then their way back to the host behind an event
+    // moments of layers [a, b) at the final level, then their way back to the host behind an event.  The downloads share
+    // the copy stream with the uploads, which were all enqueued above: a download starts once the last band is up.
     auto output = [&](int a, int b) {
         if (job.rc != RFLBM_OK || b <= a) return;
         h->zc = a; h->zn = b - a;
         h->t = (uint64_t)K; h->cur = K & 1;
         job.rc = do_moments<real>(h, d_rho, d_u);
-        cudaEventRecord(mom, h->stream);
-        cudaStreamWaitEvent(cs, mom, 0);
+        if (job.rc != RFLBM_OK) return;
+        if (!ck(cudaEventRecord(mom, h->stream), "cudaEventRecord (moments)")) return;
+        if (!ck(cudaStreamWaitEvent(cs, mom, 0), "cudaStreamWaitEvent (moments)")) return;
         const size_t off = (size_t)a * layer, len = (size_t)(b - a) * layer;
-        cudaMemcpyAsync((char*)rho_out_host + off, d_rho + off, len, cudaMemcpyDeviceToHost, cs);
+        if (!ck(cudaMemcpyAsync((char*)rho_out_host + off, d_rho + off, len, cudaMemcpyDeviceToHost, cs), "D2H rho")) return;
         for (int k = 0; k < 3; ++k)
-            cudaMemcpyAsync((char*)u_out_host + k * fb + off, d_u + k * fb + off, len, cudaMemcpyDeviceToHost, cs);
+            if (!ck(cudaMemcpyAsync((char*)u_out_host + k * fb + off, d_u + k * fb + off, len, cudaMemcpyDeviceToHost, cs), "D2H u")) return;
     };
-    if (C > MAXC) rc = fail(h, RFLBM_EINVAL, "rflbm_run_host: %d bands", C);       // cannot happen: CH >= nz / 32
-    if (rc == RFLBM_OK) {
+    if (job.rc == RFLBM_OK) {
         h->tma_rows = 8;
         if (K <= 2 * SKEW) {
             job.pass(-1, K + 1, CH, uploaded, output);              // one pass: init and all K steps behind the upload front
@@ -700,19 +711,28 @@ static int run_host_pipelined(rflbm* h, const void* rho_host, const void* u_host
             job.pass(K - SKEW, SKEW, CH, nothing, output);          // the last SKEW steps with the download behind them
         }
     }
-    rc = (rc != RFLBM_OK) ? rc : job.rc;
-    // ---- state of the handle: as after rflbm_init + rflbm_step(nsteps)
+    // ---- wait for both streams whatever happened (the caller's buffers must be quiet when the call returns)
+    const cudaError_t e1 = cudaStreamSynchronize(cs), e2 = cudaStreamSynchronize(h->stream);
+    for (int c = 0; c < n_up; ++c) cudaEventDestroy(up[c]);
+    if (start) cudaEventDestroy(start);
+    if (mom) cudaEventDestroy(mom);
+    ck(e1, "cudaStreamSynchronize (copy stream)");
+    ck(e2, "cudaStreamSynchronize");
     h->zc = 0; h->zn = h->nz;
     h->tma_rows = rows_full;
+    h->inject_fail = 0;
+    if (job.rc != RFLBM_OK) {
+        // a job that failed half way leaves levels mixed over the layers: the handle holds no state (ESTATE until the
+        // next rflbm_init / rflbm_set_populations / rflbm_run_host); the error text stays that of the first failure
+        h->inited = false;
+        h->t = 0; h->cur = 0; h->aa_phase = 0;
+        cudaGetLastError();
+        return job.rc;
+    }
+    // ---- state of the handle: as after rflbm_init + rflbm_step(nsteps)
     h->t = (uint64_t)nsteps; h->cur = nsteps & 1; h->aa_phase = 0; h->inited = true;
     after_state_change(h);
-    cudaError_t e1 = cudaStreamSynchronize(cs), e2 = cudaStreamSynchronize(h->stream);
-    for (int c = 0; c < C; ++c) cudaEventDestroy(up[c]);
-    cudaEventDestroy(start);
-    cudaEventDestroy(mom);
-    if (rc != RFLBM_OK) return rc;
-    rc = check_cuda(h, e1, "cudaStreamSynchronize (copy stream)");
-    return rc != RFLBM_OK ? rc : check_cuda(h, e2, "cudaStreamSynchronize");
+    return RFLBM_OK;
 }
 
 extern "C" int rflbm_run_host(rflbm_t* h, const void* rho_host, const void* u_host, int nsteps, void* rho_out_host,
@@ -736,6 +756,14 @@ extern "C" int rflbm_run_host(rflbm_t* h, const void* rho_host, const void* u_ho
                    ? run_host_pipelined<double>(h, rho_host, u_host, nsteps, rho_out_host, u_out_host, d_rho, d_u, fb)
                    : run_host_pipelined<float>(h, rho_host, u_host, nsteps, rho_out_host, u_out_host, d_rho, d_u, fb);
     return run_host_serial(h, rho_host, u_host, nsteps, rho_out_host, u_out_host, d_rho, d_u, fb);
+}
+
+extern "C" int rflbm_debug_inject_failure(rflbm_t* h, int nth_call)
+{
+    if (!h) return RFLBM_EINVAL;
+    if (nth_call < 0) return fail(h, RFLBM_EINVAL, "nth_call < 0");
+    h->inject_fail = nth_call;
+    return RFLBM_OK;
 }
 
 extern "C" int rflbm_set_copy_stream(rflbm_t* h, void* cuda_stream)

@@ -49,6 +49,7 @@ struct rflbm {
     const char* last_kernel;   // what the last rflbm_step launched (static string)
     int zc, zn;           // owned layers [zc, zc+zn) the next launch covers (0, nz except inside rflbm_run_host's pipeline)
     cudaStream_t copy_stream;  // optional second stream for the copies of rflbm_run_host (rflbm_set_copy_stream)
+    int inject_fail;           // test hook (rflbm_debug_inject_failure): the n-th checked CUDA call of the next pipelined job fails
     char err[512];
 };
 

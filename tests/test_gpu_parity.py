@@ -495,3 +495,38 @@ def test_two_handles_on_their_own_streams_do_not_interfere():
     torch.cuda.synchronize()
     assert torch.equal(fa, solo[0]) and torch.equal(fb, solo[1])
     assert a.launch_count == 26 and b.step_count == 24
+
+
+@pytest.mark.parametrize("nth", [1, 5, 8, 11, 29, 31, 40])
+def test_run_host_pipelined_failure_leaves_no_state(nth):
+    """ADVICE r2 / VERDICT r2 item 6: every CUDA call of the pipelined rflbm_run_host is checked; a job in which one of
+    them fails (event creation, the first record, an upload, a wait, the download side: rflbm_debug_inject_failure makes
+    the nth checked call report an error) returns ECUDA with the text of that first failure and leaves the handle
+    WITHOUT a state (ESTATE on the next rflbm_step) instead of claiming t = nsteps; both streams are quiet and no
+    sticky error is left, and the same handle then runs a proper job to the result a fresh handle gives."""
+    torch = torch_()
+    nx, ny, nz = 36, 4, 40
+    sim = binding.Rflbm(nx, ny, nz, 0.8, 1e-4, 1.0, 21)
+    sim.set_copy_stream(torch.cuda.Stream())
+    sim.init()
+    sim.step(2)
+    rho, u = synthetic.smooth_random_fields(nx, ny, nz, 12)
+    rho_h = torch.from_numpy(rho).pin_memory(); u_h = torch.from_numpy(u).pin_memory()
+    ro = torch.empty(nz, ny, nx, dtype=torch.float64).pin_memory(); uo = torch.empty(3, nz, ny, nx, dtype=torch.float64).pin_memory()
+    sim.debug_inject_failure(nth)
+    with pytest.raises(binding.RflbmError) as e:
+        sim.run_host(rho_h, u_h, 5, ro, uo)
+    assert e.value.code == binding.ECUDA and "unknown error" in str(e.value).lower()
+    with pytest.raises(binding.RflbmError) as e:
+        sim.step(1)
+    assert e.value.code == binding.ESTATE
+    with pytest.raises(binding.RflbmError) as e:
+        sim.moments()
+    assert e.value.code == binding.ESTATE
+    assert sim.step_count == 0
+    torch.cuda.synchronize()                                                   # no sticky error left behind
+    sim.run_host(rho_h, u_h, 5, ro, uo)                                        # the hook disarmed itself
+    fresh = binding.Rflbm(nx, ny, nz, 0.8, 1e-4, 1.0, 21)
+    ro2 = torch.empty_like(ro).pin_memory(); uo2 = torch.empty_like(uo).pin_memory()
+    fresh.run_host(rho_h, u_h, 5, ro2, uo2)
+    assert torch.equal(ro, ro2) and torch.equal(uo, uo2) and sim.step_count == 5

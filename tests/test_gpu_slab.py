@@ -151,3 +151,56 @@ def test_slab_resume_from_exported_state_and_set_populations():
     with pytest.raises(binding.RflbmError) as e:
         slabs[0].step(2)                                      # one step at a time in slab mode
     assert e.value.code == binding.EINVAL
+
+
+@pytest.mark.parametrize("scheme,steps", [(binding.SCHEME_AA, 1), (binding.SCHEME_AA, 2), (binding.SCHEME_AB, 1)])
+def test_second_unpack_of_a_finished_side_is_a_no_op(scheme, steps):
+    """after the exchange a repeated rflbm_halo_unpack must not launch again.  In the AA scheme after an odd
+    step (the faces carry populations HOME into the owned boundary layer) a second unpack would overwrite nine
+    populations of that layer with whatever the buffer holds by then; the slab that owns only a wall layer also
+    reports finite (zero) statistics instead of 0/0."""
+    torch = torch_()
+    nx, ny, nzg, split = 40, 5, 8, (1, 4, 3)
+    rho, u = synthetic.smooth_random_fields(nx, ny, nzg, 19)
+    slabs, z0 = [], 0
+    for nz in split:
+        s = binding.Rflbm(nx, ny, nz, 0.8, 1e-4, 1.0, 77, binding.F64, scheme=scheme, slab=(z0, nzg))
+        s.set_walls_z(True)
+        s.init(torch.from_numpy(ghosted(rho, z0, nz, nzg)), torch.from_numpy(ghosted(u, z0, nz, nzg)))
+        slabs.append(s)
+        z0 += nz
+    exchange(slabs)
+    for _ in range(steps):
+        for s in slabs:
+            s.step(1)
+        exchange(slabs)
+    before = [s.get_populations().clone() for s in slabs]
+    launches = [s.launch_count for s in slabs]
+    junk = torch.full((9, ny, nx), 123.0, dtype=torch.float64, device="cuda")
+    for s in slabs:
+        s.halo_unpack(LOW, junk)
+        s.halo_unpack(HIGH, junk)
+        assert not s.halo_pending
+    assert [s.launch_count for s in slabs] == launches
+    for s in slabs:
+        s.step(1)
+    assert all(s.halo_pending for s in slabs)
+    exchange(slabs)
+    # the junk never entered: the same three slabs stepped without the extra calls give the same bits
+    again, z0 = [], 0
+    for nz, f in zip(split, before):
+        full = torch.cat(before, dim=1)
+        idx = [(z0 - 1 + i) % nzg for i in range(nz + 2)]
+        s = binding.Rflbm(nx, ny, nz, 0.8, 1e-4, 1.0, 77, binding.F64, scheme=scheme, slab=(z0, nzg))
+        s.set_walls_z(True)
+        s.set_populations(full[:, idx].contiguous(), steps)
+        again.append(s)
+        z0 += nz
+    exchange(again)
+    for s in again:
+        s.step(1)
+    exchange(again)
+    for a, b in zip(again, slabs):
+        assert torch.equal(a.get_populations(), b.get_populations())
+    d = slabs[0].diagnostics()                                # global layer 0 only: solid, no fluid site
+    assert d == [0.0] * 10
