@@ -6,7 +6,9 @@ decomposition"): every rank owns a contiguous range of z layers of ONE global la
 (9 nx ny sizeof(real) bytes per face: 4.7 MB at 256^2 fp64).  All arithmetic stays in the CUDA kernels of csrc/
 (the step, pack and unpack kernels behind include/rflbm.h); this module only decides who owns what and moves the
 packed faces: point-to-point send/recv (NCCL between GPUs; gloo through pinned host buffers where ranks share a GPU
-or the backend is gloo), no reduction collective on the data path.  Because walls and the Philox key use the GLOBAL
+or the backend is gloo), no reduction collective on the data path.  STATUS: the gloo transport is what every test runs
+(2-3 ranks, CPU tensors and one shared GPU); the NCCL branches (FaceTransport.exchange, SlabLattice.diagnostics) are
+UNTESTED ON HARDWARE - no box with two GPUs has been available to this repository.  Because walls and the Philox key use the GLOBAL
 z, the ranks together compute, bit for bit, what one handle computes on the undivided lattice
 (tests/test_gpu_slab.py on one process, tests/test_gpu_slab_dist.py on two).
 
