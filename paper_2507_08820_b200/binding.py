@@ -43,6 +43,7 @@ SYMBOLS = {
     "rflbm_step": (_i32, [_vp, _i32]),
     "rflbm_moments": (_i32, [_vp, _vp, _vp]),
     "rflbm_stress": (_i32, [_vp, _vp]),
+    "rflbm_snapshot": (_i32, [_vp, _vp, _vp, _vp]),
     "rflbm_diagnostics": (_i32, [_vp, C.POINTER(_dbl)]),
     "rflbm_get_populations": (_i32, [_vp, _vp]),
     "rflbm_set_populations": (_i32, [_vp, _vp, _u64]),
@@ -228,6 +229,17 @@ class Rflbm:
                 pi = self.torch.empty((6,) + self.shape, dtype=self.dtype, device=self.device)
             self._ck(self.lib.rflbm_stress(self.h, pi.data_ptr()))
         return pi
+
+    def snapshot(self, rho=None, u=None, pi=None):
+        """rho, u, pi of the current state from one pass over the populations (= moments() + stress(), bit for bit)"""
+        t = self.torch
+        with self._ctx():
+            if rho is None:
+                rho = t.empty(self.shape, dtype=self.dtype, device=self.device)
+                u = t.empty((3,) + self.shape, dtype=self.dtype, device=self.device)
+                pi = t.empty((6,) + self.shape, dtype=self.dtype, device=self.device)
+            self._ck(self.lib.rflbm_snapshot(self.h, rho.data_ptr(), u.data_ptr(), pi.data_ptr()))
+        return rho, u, pi
 
     def diagnostics(self):
         out = (_dbl * 10)()

@@ -254,19 +254,21 @@ static int gather_mode(const rflbm* h)
 {
     return h->scheme == RFLBM_SCHEME_AB ? GATHER_AB : (h->aa_phase ? GATHER_AA1 : GATHER_AA0);
 }
-#define RFLBM_LAUNCH_OBSERVABLE(KERNEL, ...)                                                                      \
+#define RFLBM_LAUNCH_OBSERVABLE_GRID(GRID, KERNEL, ...)                                                           \
     do {                                                                                                          \
         const int gm_ = gather_mode(h);                                                                           \
+        const dim3 grid_ = (GRID);                                                                                \
         if (h->walls) {                                                                                           \
-            if (gm_ == GATHER_AB) KERNEL<real, true, GATHER_AB><<<zgrid(h), h->block, 0, h->stream>>>(__VA_ARGS__);       \
-            else if (gm_ == GATHER_AA1) KERNEL<real, true, GATHER_AA1><<<zgrid(h), h->block, 0, h->stream>>>(__VA_ARGS__); \
-            else KERNEL<real, true, GATHER_AA0><<<zgrid(h), h->block, 0, h->stream>>>(__VA_ARGS__);                       \
+            if (gm_ == GATHER_AB) KERNEL<real, true, GATHER_AB><<<grid_, h->block, 0, h->stream>>>(__VA_ARGS__);          \
+            else if (gm_ == GATHER_AA1) KERNEL<real, true, GATHER_AA1><<<grid_, h->block, 0, h->stream>>>(__VA_ARGS__);   \
+            else KERNEL<real, true, GATHER_AA0><<<grid_, h->block, 0, h->stream>>>(__VA_ARGS__);                          \
         } else {                                                                                                  \
-            if (gm_ == GATHER_AB) KERNEL<real, false, GATHER_AB><<<zgrid(h), h->block, 0, h->stream>>>(__VA_ARGS__);      \
-            else if (gm_ == GATHER_AA1) KERNEL<real, false, GATHER_AA1><<<zgrid(h), h->block, 0, h->stream>>>(__VA_ARGS__); \
-            else KERNEL<real, false, GATHER_AA0><<<zgrid(h), h->block, 0, h->stream>>>(__VA_ARGS__);                      \
+            if (gm_ == GATHER_AB) KERNEL<real, false, GATHER_AB><<<grid_, h->block, 0, h->stream>>>(__VA_ARGS__);         \
+            else if (gm_ == GATHER_AA1) KERNEL<real, false, GATHER_AA1><<<grid_, h->block, 0, h->stream>>>(__VA_ARGS__);  \
+            else KERNEL<real, false, GATHER_AA0><<<grid_, h->block, 0, h->stream>>>(__VA_ARGS__);                         \
         }                                                                                                         \
     } while (0)
+#define RFLBM_LAUNCH_OBSERVABLE(KERNEL, ...) RFLBM_LAUNCH_OBSERVABLE_GRID(zgrid(h), KERNEL, __VA_ARGS__)
 
 // slab mode: what the next halo exchange has to carry
 //   A-B, and AA after an even step: the ghost layers must receive the neighbours' face populations before the next
@@ -475,10 +477,29 @@ extern "C" int rflbm_stress(rflbm_t* h, void* pi_dev)
 }
 
 template <typename real>
+static int do_snapshot(rflbm* h, void* rho, void* u, void* pi)
+{
+    const FieldParams<real> P = field_params<real>(h);
+    RFLBM_LAUNCH_OBSERVABLE(snapshot_kernel, (const real*)h->buf[h->cur], (real*)rho, (real*)u, (real*)pi, P);
+    return after_launch(h, "snapshot_kernel");
+}
+
+extern "C" int rflbm_snapshot(rflbm_t* h, void* rho_dev, void* u_dev, void* pi_dev)
+{
+    if (!h) return RFLBM_EINVAL;
+    if (!rho_dev || !u_dev || !pi_dev) return fail(h, RFLBM_EINVAL, "rho_dev / u_dev / pi_dev is NULL");
+    if (!h->inited) return fail(h, RFLBM_ESTATE, "rflbm_snapshot before init");
+    RFLBM_REQUIRE_HALO(h);
+    return (h->precision == RFLBM_F64) ? do_snapshot<double>(h, rho_dev, u_dev, pi_dev) : do_snapshot<float>(h, rho_dev, u_dev, pi_dev);
+}
+
+template <typename real>
 static int do_diagnostics(rflbm* h)
 {
     const FieldParams<real> P = field_params<real>(h);
-    RFLBM_LAUNCH_OBSERVABLE(diagnostics_kernel, (const real*)h->buf[h->cur], h->acc, P);
+    // every block walks the layers z = blockIdx.z, blockIdx.z + DIAG_ZBLOCKS, ... of its (x, y) patch
+    const dim3 grid(h->grid.x, h->grid.y, (unsigned)std::min(h->zn, (int)DIAG_ZBLOCKS));
+    RFLBM_LAUNCH_OBSERVABLE_GRID(grid, diagnostics_kernel, (const real*)h->buf[h->cur], h->acc, P, h->zn);
     return after_launch(h, "diagnostics_kernel");
 }
 
@@ -488,15 +509,21 @@ extern "C" int rflbm_diagnostics(rflbm_t* h, double out_host[10])
     if (!out_host) return fail(h, RFLBM_EINVAL, "out_host is NULL");
     if (!h->inited) return fail(h, RFLBM_ESTATE, "rflbm_diagnostics before init");
     RFLBM_REQUIRE_HALO(h);
-    int rc = check_cuda(h, cudaMemsetAsync(h->acc, 0, 10 * sizeof(double), h->stream), "cudaMemsetAsync");
+    static_assert(DIAG_ROWS * DIAG_PITCH * sizeof(double) == 4096, "the diagnostics rows fill the 4 KiB scratch");
+    int rc = check_cuda(h, cudaMemsetAsync(h->acc, 0, 4096, h->stream), "cudaMemsetAsync");
     if (rc != RFLBM_OK) return rc;
     rc = (h->precision == RFLBM_F64) ? do_diagnostics<double>(h) : do_diagnostics<float>(h);
     if (rc != RFLBM_OK) return rc;
-    double s[10];
-    rc = check_cuda(h, cudaMemcpyAsync(s, h->acc, sizeof(s), cudaMemcpyDeviceToHost, h->stream), "cudaMemcpyAsync");
+    double rows[DIAG_ROWS * DIAG_PITCH];
+    rc = check_cuda(h, cudaMemcpyAsync(rows, h->acc, sizeof(rows), cudaMemcpyDeviceToHost, h->stream), "cudaMemcpyAsync");
     if (rc != RFLBM_OK) return rc;
     rc = check_cuda(h, cudaStreamSynchronize(h->stream), "cudaStreamSynchronize");
     if (rc != RFLBM_OK) return rc;
+    double s[10];
+    for (int n = 0; n < 10; ++n) {
+        s[n] = 0.0;
+        for (int r = 0; r < DIAG_ROWS; ++r) s[n] += rows[r * DIAG_PITCH + n];
+    }
     // fluid layers owned by this handle (solid layers are global z = 0 and nz_global - 1)
     const int z0 = h->slab ? h->z0 : 0, nzg = h->slab ? h->nzg : h->nz;
     const int nfl = h->nz - (h->walls ? (z0 == 0) + (z0 + h->nz == nzg) : 0);

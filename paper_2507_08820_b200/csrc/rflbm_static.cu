@@ -105,10 +105,10 @@ static_partial_kernel(const real* __restrict__ f, double* __restrict__ partial, 
 #pragma unroll
         for (int i = 0; i < Q; ++i) g[canon_cz(i) + 1][canon_cy(i) + 1][canon_cx(i) + 1] = __ldg(f + (long long)i * P.N + s);
         const Moments10<real> m = forward_moments(g);
-        const double rho = (double)m.rho;
-        const double ux = (double)m.jx / rho + P.hg[0];
-        const double uy = (double)m.jy / rho + P.hg[1];
-        const double uz = (double)m.jz / rho + P.hg[2];
+        const double rho = (double)m.rho, inv = 1.0 / rho;     // one fp64 division per site, not three
+        const double ux = fma((double)m.jx, inv, P.hg[0]);
+        const double uy = fma((double)m.jy, inv, P.hg[1]);
+        const double uz = fma((double)m.jz, inv, P.hg[2]);
         v[0] += rho; v[1] += rho * ux; v[2] += rho * uy; v[3] += rho * uz;
         v[4] += ux; v[5] += uy; v[6] += uz; v[7] += ux * ux; v[8] += uy * uy; v[9] += uz * uz;
     }

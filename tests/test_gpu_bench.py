@@ -42,12 +42,17 @@ def test_bench_line_has_the_contract_keys():
     assert c["out_of_cache"]["value"] > 0
     s = d["sustained"]
     assert s["steps"] >= 5 and s["ms_per_step"] > 0 and "clocks" in s
+    # the sustained fraction is readable from `roofline` alone, with the clocks it was held at
+    assert r["frac_sustained"] == s["frac"] and r["achieved_sustained"] == s["hbm_gbs"] and r["sustained_clocks"] == s["clocks"]
+    assert abs(r["frac_sustained"] - 2 * 27 * 8 * 64 ** 3 / (s["ms_per_step"] * 1e-3) / 1e9 / r["peak"]) < 1e-9
+    assert "burst" in r["frac_is"] and r["sustained_steps"] == s["steps"]
+    assert e["outputs_equal_device_moments"] is True
     assert d["mass_rel_err"] < 1e-12
 
 
 def test_bench_aux_and_slab_modes():
     a = run_bench("--aux", "--size", "64")["aux"]
-    assert set(a) == {"rflbm_moments", "rflbm_stress", "rflbm_diagnostics", "rflbm_get_populations",
+    assert set(a) == {"rflbm_moments", "rflbm_stress", "rflbm_snapshot", "rflbm_diagnostics", "rflbm_get_populations",
                       "rflbm_set_populations", "rflbm_init(rho,u)", "rflbm_init(NULL)"}
     assert all(v["ms"] > 0 and v["gbs"] > 0 for v in a.values())
     d = run_bench("--size", "64", "--steps", "4", "--warmup", "3", "--no-cpu", "--no-sustained", "--decomp", "slab")

@@ -370,6 +370,37 @@ def test_stress_observable_matches_oracle(prec, walls):
     assert d < (1e-12 if prec == binding.F64 else 1e-5), d
 
 
+@pytest.mark.parametrize("shape,prec,scheme,walls,steps", [
+    ((40, 9, 6), binding.F64, binding.SCHEME_AB, False, 15), ((130, 7, 5), binding.F64, binding.SCHEME_AA, True, 3),
+    ((130, 7, 5), binding.F32, binding.SCHEME_AA, True, 4), ((33, 33, 3), binding.F32, binding.SCHEME_AB, True, 6),
+    ((5, 3, 2), binding.F64, binding.SCHEME_AB, False, 2)])
+def test_snapshot_equals_moments_plus_stress_bit_for_bit(shape, prec, scheme, walls, steps):
+    """rflbm_snapshot (rho, rho u and Pi_ab saved together) is one gather with ten stores; it must write
+    exactly what rflbm_moments and rflbm_stress write - which the tests above tie to the oracle - in both schemes and AA
+    phases, with walls (solid layers: zeros) and a body force (u carries g/2), and launch one kernel."""
+    torch = torch_()
+    nx, ny, nz = shape
+    sim = binding.Rflbm(nx, ny, nz, 0.8, 1e-4, 1.0, 13, prec, scheme=scheme)
+    if walls:
+        sim.set_walls_z(True)
+        sim.set_force(1e-6, -3e-6, 0.0)
+    rho, u = synthetic.smooth_random_fields(nx, ny, nz, 6)
+    sim.init(torch.from_numpy(rho), torch.from_numpy(u))
+    sim.step(steps)
+    r1, u1 = sim.moments()
+    p1 = sim.stress()
+    n0 = sim.launch_count
+    r2, u2, p2 = sim.snapshot()
+    assert sim.launch_count == n0 + 1
+    assert torch.equal(r1, r2) and torch.equal(u1, u2) and torch.equal(p1, p2)
+    if walls:
+        assert float(r2[0].abs().max()) == 0.0 and float(p2[:, -1].abs().max()) == 0.0
+    fresh = binding.Rflbm(4, 4, 4, 1.0, 0.0)
+    with pytest.raises(binding.RflbmError) as e:
+        fresh.snapshot()
+    assert e.value.code == binding.ESTATE
+
+
 @pytest.mark.parametrize("shape,prec,walls,force,kT,variant", [
     ((16, 16, 16), binding.F64, False, None, 1e-4, binding.KERNEL_AUTO),
     ((5, 7, 9), binding.F64, True, (1e-5, -2e-6, 3e-6), 1e-4, binding.KERNEL_AUTO),
