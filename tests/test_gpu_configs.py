@@ -327,8 +327,7 @@ def test_fig1_fig2_fluctuation_spectra_256(tau):
     pi = torch.empty((6, n, n, n), dtype=torch.float64, device="cuda")
     nsamp = 0
     while sim.step_count <= 2000:
-        sim.moments(rho, u)
-        sim.stress(pi)
+        sim.snapshot(rho, u, pi)                       # the paper's snapshot (:252) in one pass: = moments + stress bit for bit
         fields = [("rho", rho, 3 * kT)] + [("j", rho * u[a], kT) for a in range(3)] + \
                  [("pd", pi[a], 2.0 / 3.0 * kT) for a in range(3)] + [("po", pi[a], 1.0 / 3.0 * kT) for a in range(3, 6)]
         for name, fld, norm in fields:
