@@ -1,5 +1,5 @@
-// rflbm_step_tma.cuh — the hot kernel, TMA-staged (sm_100a): one time step of Eq.24 on an fp64 lattice with
-// nx >= 128, nx even.
+// rflbm_step_tma.cuh — the hot kernel, TMA-staged (sm_100a): one time step of Eq.24 on an fp64 or fp32 lattice with
+// any nx >= 32 (tiles of 128, 64 or 32 sites; the internal row pitch is padded to whole 128-byte lines).
 //
 // Why (profiles/r01a_*): in the plain one-thread-per-site kernel every one of the 27 neighbour loads costs 4-5
 // integer instructions of per-thread 64-bit address arithmetic, and a block's memory latency is exposed between
