@@ -63,6 +63,17 @@ typedef CUresult (*encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_
                                     const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                     CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
+// L2 promotion of the tensor maps, per precision (compile-time).  NONE: measured against L2_256B (rounds 1-2) and L2_128B
+// in one call at 512^3, sustained (profiles/r03_variants.md): fp64 9.69 -> 9.64-9.65 ms, fp32 4.986 -> 4.981 ms, fp32
+// L2 read sectors -10 %, DRAM reads 1.053 -> 1.036 x algorithmic (a box is 16 bytes wider than its tile on either side;
+// promotion turned those two half sectors into two 256-byte fetches).
+#ifndef RFLBM_TMAP_PROMO_F64
+#define RFLBM_TMAP_PROMO_F64 CU_TENSOR_MAP_L2_PROMOTION_NONE
+#endif
+#ifndef RFLBM_TMAP_PROMO_F32
+#define RFLBM_TMAP_PROMO_F32 CU_TENSOR_MAP_L2_PROMOTION_NONE
+#endif
+
 // 4-D view [nzs][ny][27][nx] (x pitch px) of one population buffer, box = BOX_X consecutive x of BOX_Q populations of one row
 static bool make_tensor_map(rflbm* h, void* base, CUtensorMap* out, bool store_box = false)
 {
@@ -82,7 +93,7 @@ static bool make_tensor_map(rflbm* h, void* base, CUtensorMap* out, bool store_b
     const cuuint32_t estr[4] = {1, 1, 1, 1};
     const CUresult r = ((encode_tiled_fn)fn)(out, f64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, base, dims, strides, box, estr,
                                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                                             CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                                             f64 ? RFLBM_TMAP_PROMO_F64 : RFLBM_TMAP_PROMO_F32, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS;
 }
 

@@ -157,6 +157,9 @@ __device__ __forceinline__ void issue_tile(const CUtensorMap* tmap, uint32_t s_i
 // warps per scheduler), so fp64 keeps its per-thread streaming stores.  Issuing the box one row late, behind the next
 // block barrier: fp64 +2 %, fp32 +0.6 % slower than the immediate form.  The odd AA phase cannot use a box at all (its
 // cx = +-1 populations move by one element: box starts must be multiples of 16 bytes).
+#ifndef RFLBM_F64_AB_BLOCKS
+#define RFLBM_F64_AB_BLOCKS 3        // resident blocks per SM of the fp64 A-B instantiation (see the comment below)
+#endif
 template <typename real, int PHASE> __host__ __device__ constexpr bool tma_store() { return sizeof(real) == 4 && PHASE != STEP_AA_ODD; }
 template <typename real, int PHASE> __host__ __device__ constexpr int tma_store_bytes()
 {
@@ -167,7 +170,7 @@ template <typename real, int PHASE> __host__ __device__ constexpr int tma_store_
 // one call, sustained: 9.73 vs 9.80 and 9.86 vs 9.92 ms (24 fewer instructions per site, no spills; 5 blocks of 96
 // registers: 10.13).  The in-place phases keep 4 blocks (10.09 vs 10.14 with 3).  fp32: 64 registers, 15 KB -> 8 blocks.
 template <typename real, int TX, bool WALLS, bool FORCE, bool NOISE, bool BGK, bool GHOST, int PHASE>
-__global__ void __launch_bounds__(BLOCK_T, sizeof(real) == 8 ? (PHASE == STEP_AB ? 3 : 4) : (tma_store<real, PHASE>() ? 6 : 8))
+__global__ void __launch_bounds__(BLOCK_T, sizeof(real) == 8 ? (PHASE == STEP_AB ? RFLBM_F64_AB_BLOCKS : 4) : (tma_store<real, PHASE>() ? 6 : 8))
 step_kernel_tma(const __grid_constant__ CUtensorMap tmap_src, const __grid_constant__ CUtensorMap tmap_dst, const real* src, real* dst,
                 const __grid_constant__ StepParams<real> P, int rows)
 {
